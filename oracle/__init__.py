@@ -1,0 +1,150 @@
+"""ctypes wrapper around the CPU oracle (oracle/ps_oracle.c).
+
+TEST INFRASTRUCTURE, NOT PRODUCT: only tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / `--impl reference` legs may import this package.  Nothing under
+paper_2104_01636_b200/ imports it, and it imports nothing from there.
+
+`build()` compiles the C file with `gcc -O2 -ffp-contract=off -fopenmp` (no FMA contraction, no
+fast-math).  Arrays are float64, C-contiguous, shape (nz, ny, nx).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from dataclasses import dataclass
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "ps_oracle.c")
+_HDR = os.path.join(_HERE, "ps_oracle.h")
+_LIB = os.path.join(_HERE, "libps_oracle.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile oracle/ps_oracle.c -> oracle/libps_oracle.so (no-op if up to date)."""
+    if (not force and os.path.exists(_LIB)
+            and os.path.getmtime(_LIB) >= max(os.path.getmtime(_SRC), os.path.getmtime(_HDR))):
+        return _LIB
+    tmp = f"{_LIB}.{os.getpid()}.tmp"
+    cmd = ["gcc", "-std=c11", "-O2", "-ffp-contract=off", "-fno-fast-math", "-fopenmp", "-fPIC",
+           "-shared", "-Wall", "-Wextra", "-o", tmp, _SRC, "-lm"]
+    subprocess.run(cmd, check=True, cwd=_HERE)
+    os.replace(tmp, _LIB)
+    return _LIB
+
+
+class _Info(ctypes.Structure):
+    _fields_ = [("sweeps", ctypes.c_int), ("converged", ctypes.c_int),
+                ("res_abs", ctypes.c_double), ("res_rel", ctypes.c_double),
+                ("rhs_norm", ctypes.c_double)]
+
+
+@dataclass
+class Info:
+    sweeps: int
+    converged: bool
+    res_abs: float
+    res_rel: float
+    rhs_norm: float
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(build())
+        dp, i, d, sz = ctypes.POINTER(ctypes.c_double), ctypes.c_int, ctypes.c_double, ctypes.c_size_t
+        lib.ora_density.argtypes = [sz, dp, d, d, dp]
+        lib.ora_coefficients.argtypes = [i, i, i, d, d, d, dp, dp, dp, dp]
+        lib.ora_half_sweep.argtypes = [i, i, i, dp, dp, dp, dp, dp, d, i]
+        lib.ora_sweep.argtypes = [i, i, i, dp, dp, dp, dp, dp, d]
+        lib.ora_apply.argtypes = [i, i, i, dp, dp, dp, dp, dp]
+        lib.ora_residual.argtypes = [i, i, i, dp, dp, dp, dp, dp, dp, dp, dp]
+        lib.ora_solve.argtypes = [i, i, i, dp, dp, dp, dp, dp, d, i, d, i, ctypes.POINTER(_Info)]
+        for f in ("ora_density", "ora_coefficients", "ora_half_sweep", "ora_sweep", "ora_apply",
+                  "ora_residual", "ora_solve"):
+            getattr(lib, f).restype = None
+        _lib = lib
+    return _lib
+
+
+def _p(a: np.ndarray):
+    assert a.dtype == np.float64 and a.flags["C_CONTIGUOUS"], "float64 C-contiguous expected"
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+
+
+def _shape(a: np.ndarray):
+    nz, ny, nx = a.shape
+    return nx, ny, nz
+
+
+def density(F: np.ndarray, rho_l: float, rho_g: float) -> np.ndarray:
+    F = np.ascontiguousarray(F, dtype=np.float64)
+    rho = np.empty_like(F)
+    _load().ora_density(F.size, _p(F), rho_l, rho_g, _p(rho))
+    return rho
+
+
+def coefficients(F: np.ndarray, rho_l: float, rho_g: float, dx: float, dy: float, dz: float):
+    """O1 + O2: returns (ax, ay, az), each shaped like F."""
+    rho = density(F, rho_l, rho_g)
+    nx, ny, nz = _shape(rho)
+    ax, ay, az = np.empty_like(rho), np.empty_like(rho), np.empty_like(rho)
+    _load().ora_coefficients(nx, ny, nz, dx, dy, dz, _p(rho), _p(ax), _p(ay), _p(az))
+    return ax, ay, az
+
+
+def half_sweep(coef, rhs: np.ndarray, p: np.ndarray, omega: float, colour: int) -> None:
+    ax, ay, az = coef
+    nx, ny, nz = _shape(p)
+    _load().ora_half_sweep(nx, ny, nz, _p(ax), _p(ay), _p(az), _p(rhs), _p(p), omega, colour)
+
+
+def sweep(coef, rhs: np.ndarray, p: np.ndarray, omega: float, count: int = 1) -> None:
+    ax, ay, az = coef
+    nx, ny, nz = _shape(p)
+    lib = _load()
+    for _ in range(count):
+        lib.ora_sweep(nx, ny, nz, _p(ax), _p(ay), _p(az), _p(rhs), _p(p), omega)
+
+
+def apply(coef, p: np.ndarray) -> np.ndarray:
+    ax, ay, az = coef
+    nx, ny, nz = _shape(p)
+    out = np.empty_like(p)
+    _load().ora_apply(nx, ny, nz, _p(ax), _p(ay), _p(az), _p(p), _p(out))
+    return out
+
+
+def residual(coef, rhs: np.ndarray, p: np.ndarray):
+    """O5: returns (res_abs, res_rel, rhs_norm)."""
+    ax, ay, az = coef
+    nx, ny, nz = _shape(p)
+    ra, rr, bn = ctypes.c_double(), ctypes.c_double(), ctypes.c_double()
+    _load().ora_residual(nx, ny, nz, _p(ax), _p(ay), _p(az), _p(rhs), _p(p),
+                         ctypes.byref(ra), ctypes.byref(rr), ctypes.byref(bn))
+    return ra.value, rr.value, bn.value
+
+
+def solve(coef, rhs: np.ndarray, p: np.ndarray, omega: float, max_sweeps: int, tol: float,
+          check_interval: int = 50) -> Info:
+    """O6 in place on p."""
+    ax, ay, az = coef
+    nx, ny, nz = _shape(p)
+    info = _Info()
+    _load().ora_solve(nx, ny, nz, _p(ax), _p(ay), _p(az), _p(rhs), _p(p), omega, max_sweeps,
+                      tol, check_interval, ctypes.byref(info))
+    return Info(info.sweeps, bool(info.converged), info.res_abs, info.res_rel, info.rhs_norm)
+
+
+def threads() -> int:
+    """OpenMP threads the half-sweeps use (OMP_NUM_THREADS or all cores)."""
+    env = os.environ.get("OMP_NUM_THREADS")
+    if env:
+        return int(env)
+    try:
+        return len(os.sched_getaffinity(0))
+    except AttributeError:
+        return os.cpu_count() or 1

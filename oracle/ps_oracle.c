@@ -1,0 +1,176 @@
+/*
+ * ps_oracle.c -- CPU oracle for the variable-coefficient pressure-Poisson red-black SOR path.
+ *
+ * TEST INFRASTRUCTURE, NOT PRODUCT.  Only tests/, __graft_entry__.smoke() and bench.py's
+ * cpu_baseline / --impl reference legs may build, load or call this file.  It shares no code,
+ * header, table or helper with the CUDA path under paper_2104_01636_b200/csrc/.
+ *
+ * What it is: the method is an ITERATION, so the oracle is the algorithm written out step by
+ * step in the order of SURVEY.md §8.c O1-O6, plain triple loops, fp64, no blocking, no fusion,
+ * no reordering.  Build: gcc -O2 -ffp-contract=off (no FMA contraction, no fast-math), so every
+ * expression below rounds exactly as written.
+ *
+ * Paper passages followed (citations are lines of /root/reference/PAPER.md):
+ *   O1 density           rho = alpha*rho_l + (1-alpha)*rho_g        PAPER.md:66 eq (4), :92 step 4
+ *   O2 face coefficient  linear averaging c->f of rho, then 1/rho_f PAPER.md:117; operator :111
+ *      boundaries        no-penetration walls in x,y; periodic z
+ *      grid              uniform Cartesian collocated
+ *   O3/O4 red-black SOR  "red black SOR relaxation scheme"
+ *   O5/O6 residual, L2 norms, stopping rule: the paper is silent; BASELINE.json north_star and
+ *      DESIGN.md readings S1-S10 fix them.
+ *
+ * Pins (tests/test_oracle_pins.py, tests/golden/): closed-form eigenvalues of the constant-rho
+ * operator (P1), dense LU on 4x4x8 (P2), symmetry (P3), flux telescoping / compatibility (P4),
+ * 1-D periodic variable-coefficient closed form (P5), Gauss-Seidel zero residual on the updated
+ * colour (P6), even z-shift bitwise invariance (P7), power-of-two scaling (P8), Young's SOR rate
+ * (P9), energy monotonicity (P10).  Every function here is pinned by at least one of them.
+ *
+ * Layout: n = i + nx*(j + ny*k), x fastest, z slowest; all fields double.
+ * Sign convention: (A p)_c = sum_f a_f (p_nb - p_c) = s - d*p_c; A p = rhs.
+ */
+#include <math.h>
+#include <stddef.h>
+
+#include "ps_oracle.h"
+
+#define IDX(i, j, k) ((size_t)(i) + (size_t)nx * ((size_t)(j) + (size_t)ny * (size_t)(k)))
+
+/* O1: eq (4).  F is the LIQUID volume fraction alpha. */
+void ora_density(size_t n, const double *F, double rho_l, double rho_g, double *rho)
+{
+    for (size_t c = 0; c < n; ++c)
+        rho[c] = (rho_l * F[c]) + (rho_g * (1.0 - F[c]));
+}
+
+/* O2: +x, +y, +z face coefficient of every cell, (1/h^2)/rho_f with rho_f the arithmetic mean of
+ * the two cell densities ("linear averaging procedure to compute face value (eg.
+ * rho_f ...)").  Wall faces are 0; z wraps ("periodic"). */
+void ora_coefficients(int nx, int ny, int nz, double dx, double dy, double dz,
+                      const double *rho, double *ax, double *ay, double *az)
+{
+    const double cx = 1.0 / (dx * dx), cy = 1.0 / (dy * dy), cz = 1.0 / (dz * dz);
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) {
+                const size_t n = IDX(i, j, k);
+                ax[n] = (i < nx - 1) ? cx / (0.5 * (rho[n] + rho[IDX(i + 1, j, k)])) : 0.0;
+                ay[n] = (j < ny - 1) ? cy / (0.5 * (rho[n] + rho[IDX(i, j + 1, k)])) : 0.0;
+                az[n] = cz / (0.5 * (rho[n] + rho[IDX(i, j, (k + 1) % nz)]));
+            }
+}
+
+/* The six face coefficients and neighbour values of cell (i,j,k), and the two sums of O3:
+ *   s = sum_f a_f p_nb   (12 roundings, left to right)      d = sum_f a_f
+ * A wall neighbour is read at the clamped index and multiplied by the 0.0 coefficient. */
+static inline void stencil_sums(int nx, int ny, int nz, const double *ax, const double *ay,
+                                const double *az, const double *p, int i, int j, int k,
+                                double *s_out, double *d_out)
+{
+    const int km = (k - 1 + nz) % nz, kp = (k + 1) % nz;
+    const double axm = (i > 0) ? ax[IDX(i - 1, j, k)] : 0.0;
+    const double axp = ax[IDX(i, j, k)];
+    const double aym = (j > 0) ? ay[IDX(i, j - 1, k)] : 0.0;
+    const double ayp = ay[IDX(i, j, k)];
+    const double azm = az[IDX(i, j, km)];
+    const double azp = az[IDX(i, j, k)];
+    const double pxm = p[IDX(i > 0 ? i - 1 : 0, j, k)];
+    const double pxp = p[IDX(i < nx - 1 ? i + 1 : nx - 1, j, k)];
+    const double pym = p[IDX(i, j > 0 ? j - 1 : 0, k)];
+    const double pyp = p[IDX(i, j < ny - 1 ? j + 1 : ny - 1, k)];
+    const double pzm = p[IDX(i, j, km)];
+    const double pzp = p[IDX(i, j, kp)];
+    *s_out = ((((axm * pxm + axp * pxp) + aym * pym) + ayp * pyp) + azm * pzm) + azp * pzp;
+    *d_out = ((((axm + axp) + aym) + ayp) + azm) + azp;
+}
+
+/* O3: one half-sweep over the cells with ((i+j+k)&1) == colour ("red black SOR").
+ * Cells of one colour never read each other, so the traversal order is free; OpenMP splits
+ * the z planes and the result does not depend on the thread count. */
+void ora_half_sweep(int nx, int ny, int nz, const double *ax, const double *ay, const double *az,
+                    const double *rhs, double *p, double omega, int colour)
+{
+#pragma omp parallel for schedule(static)
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = (j + k + colour) & 1; i < nx; i += 2) {
+                double s, d;
+                stencil_sums(nx, ny, nz, ax, ay, az, p, i, j, k, &s, &d);
+                const size_t n = IDX(i, j, k);
+                const double g = (s - rhs[n]) / d;
+                p[n] = p[n] + omega * (g - p[n]);
+            }
+}
+
+/* O4: one sweep = red ((i+j+k) even) first, then black. */
+void ora_sweep(int nx, int ny, int nz, const double *ax, const double *ay, const double *az,
+               const double *rhs, double *p, double omega)
+{
+    ora_half_sweep(nx, ny, nz, ax, ay, az, rhs, p, omega, 0);
+    ora_half_sweep(nx, ny, nz, ax, ay, az, rhs, p, omega, 1);
+}
+
+/* (A p)_c = s - d p_c: the discrete div(grad p / rho) of PAPER.md:111 (used by the pins). */
+void ora_apply(int nx, int ny, int nz, const double *ax, const double *ay, const double *az,
+               const double *p, double *Ap)
+{
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) {
+                double s, d;
+                stencil_sums(nx, ny, nz, ax, ay, az, p, i, j, k, &s, &d);
+                const size_t n = IDX(i, j, k);
+                Ap[n] = s - d * p[n];
+            }
+}
+
+/* O5: r_c = rhs_c - (A p)_c; R2 = sum r^2, B2 = sum rhs^2, accumulated in long double in
+ * linear-index order (serial on purpose). */
+void ora_residual(int nx, int ny, int nz, const double *ax, const double *ay, const double *az,
+                  const double *rhs, const double *p, double *res_abs, double *res_rel,
+                  double *rhs_norm)
+{
+    long double R2 = 0.0L, B2 = 0.0L;
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) {
+                double s, d;
+                stencil_sums(nx, ny, nz, ax, ay, az, p, i, j, k, &s, &d);
+                const size_t n = IDX(i, j, k);
+                const double r = rhs[n] - (s - d * p[n]);
+                R2 += (long double)r * (long double)r;
+                B2 += (long double)rhs[n] * (long double)rhs[n];
+            }
+    const double ra = (double)sqrtl(R2), bn = (double)sqrtl(B2);
+    *res_abs = ra;
+    *rhs_norm = bn;
+    *res_rel = (bn > 0.0) ? ra / bn : ra;
+}
+
+/* O6: sweeps s = 1..max_sweeps from the caller's p; if tol > 0 the residual is checked when
+ * s % check_interval == 0 or s == max_sweeps and the loop stops at the first check with
+ * ||r||/||rhs|| <= tol.  tol <= 0: exactly max_sweeps sweeps, norm computed once at the end. */
+void ora_solve(int nx, int ny, int nz, const double *ax, const double *ay, const double *az,
+               const double *rhs, double *p, double omega, int max_sweeps, double tol,
+               int check_interval, ora_info *info)
+{
+    double ra = 0.0, rr = 0.0, bn = 0.0;
+    int s = 0, converged = 0, checked = 0;
+    for (s = 1; s <= max_sweeps; ++s) {
+        ora_sweep(nx, ny, nz, ax, ay, az, rhs, p, omega);
+        if (tol > 0.0 && (s % check_interval == 0 || s == max_sweeps)) {
+            ora_residual(nx, ny, nz, ax, ay, az, rhs, p, &ra, &rr, &bn);
+            checked = 1;
+            if (rr <= tol) { converged = 1; break; }
+        } else {
+            checked = 0;
+        }
+    }
+    if (s > max_sweeps) s = max_sweeps;
+    if (!checked) ora_residual(nx, ny, nz, ax, ay, az, rhs, p, &ra, &rr, &bn);
+    if (tol > 0.0 && rr <= tol) converged = 1;
+    info->sweeps = s;
+    info->converged = converged;
+    info->res_abs = ra;
+    info->res_rel = rr;
+    info->rhs_norm = bn;
+}
