@@ -1,0 +1,340 @@
+#!/usr/bin/env python
+"""bench.py -- the headline measurement: red-black SOR throughput of the pressure-Poisson path.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 4]
+
+A "step" is one pass of the whole hot path over one synthetic duct:
+coefficient build from F (ps_set_fraction), `sweeps` red-black SOR sweeps and the closing
+residual/norm reduction (ps_solve with tol = 0).  Workload at N = 1: BASELINE.json configs[3],
+the 256x256x512 duct with 864 bubbles on which `metric` is quoted (500 sweeps per step).
+
+  value        Gcell-updates/s = cells * sweeps * steps / device time, inputs resident in HBM,
+               CUDA events on the launching stream, barrier + synchronize on both sides,
+               max over ranks.  N > 1: independent replicas (no data-path collective), one solve
+               per GPU on its own seeded duct, value = sum of updates / max time ("weak").
+  e2e          the same metric through ps_solve_host with pinned HOST buffers: H2D of F, rhs, p
+               and D2H of p inside the timed region, every step.
+  roofline     the sweep kernel: algorithmic bytes per launch / average launch duration measured
+               live (CUDA events around the sweep launches inside the timed steps), against the
+               measured HBM copy bandwidth of MEASURED_PEAKS.json.
+  cpu_baseline the CPU oracle, as it stands, timed on the host cores on a bounded sample.
+
+`--impl reference` times the oracle itself (there is no reference implementation to install;
+the paper has no code -- DESIGN.md "Reference arm").
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "poisson_sor_gcell_updates_per_s"
+UNIT = "Gcell-updates/s"
+# algorithmic bytes per cell per sweep-kernel launch:
+#   twopass: one colour per launch, M1 = 40 B/cell/launch (80 B per cell-update)
+#   fused:   one sweep per launch,  M2 = 48 B/cell/launch (48 B per cell-update)
+#   fused_t2: two sweeps per launch, still 48 B/cell/launch (24 B per cell-update)
+ALGO_BYTES_PER_CELL_LAUNCH = {"twopass": 40.0, "fused": 48.0, "fused_t2": 48.0}
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json config 1..5 (default 4)")
+    ap.add_argument("--sweeps", type=int, default=0, help="sweeps per step (default: the config's)")
+    ap.add_argument("--kernel", default="auto", choices=["auto", "twopass", "fused", "fused_t2"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="oracle sample budget")
+    return ap.parse_args()
+
+
+def sweeps_for(cfg: int, override: int) -> int:
+    from paper_2104_01636_b200 import workload as wl
+    if override > 0:
+        return override
+    fixed = wl.CONFIGS[cfg][7]
+    return fixed if fixed > 0 else 500
+
+
+# --------------------------------------------------------------------------- clocks
+class ClockSampler:
+    """nvidia-smi sampled every 200 ms during the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                 "--format=csv,noheader,nounits", "-lms", "200"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        self.thread.join(timeout=2)
+        sm, mx, pw, reasons = [], [], [], set()
+        for r in self.rows:
+            if len(r) < 7:
+                continue
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown",
+                                "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm),
+                "reasons": sorted(reasons)}
+
+
+def measured_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except (OSError, KeyError, ValueError):
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def ncu_traffic(kernel: str, cfg: int):
+    """DRAM bytes per launch of the sweep kernel from the committed ncu summary, or None."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            return json.load(f).get(f"{kernel}:config{cfg}")
+    except (OSError, ValueError):
+        return None
+
+
+# --------------------------------------------------------------------------- oracle legs
+def oracle_sample(w, budget_s: float):
+    """Time the CPU oracle (coefficients + n sweeps + residual) on a bounded number of sweeps."""
+    import numpy as np
+    import oracle
+    oracle.build()
+    t0 = time.perf_counter()
+    coef = oracle.coefficients(w.F, w.rho_l, w.rho_g, w.dx, w.dy, w.dz)
+    p = np.zeros_like(w.rhs)
+    oracle.sweep(coef, w.rhs, p, w.omega, 1)
+    t1 = time.perf_counter() - t0
+    n = max(1, int((budget_s - t1) / max(t1, 1e-6)))
+    t0 = time.perf_counter()
+    coef = oracle.coefficients(w.F, w.rho_l, w.rho_g, w.dx, w.dy, w.dz)
+    p = np.zeros_like(w.rhs)
+    oracle.sweep(coef, w.rhs, p, w.omega, n)
+    oracle.residual(coef, w.rhs, p)
+    dt = time.perf_counter() - t0
+    return {"value": w.cells * n / dt / 1e9, "unit": UNIT, "cores": oracle.threads(),
+            "kind": "oracle",
+            "sample": f"{w.name}: coefficient build + {n} sweeps + residual ({dt:.1f} s)"}
+
+
+def run_reference(args, rank):
+    """--impl reference: the oracle on the host cores, same config/metric, bounded steps."""
+    from paper_2104_01636_b200 import workload as wl
+    if rank.rank != 0:
+        return
+    import numpy as np
+    import oracle
+    oracle.build()
+    w = wl.make_config(args.config)
+    full = sweeps_for(args.config, args.sweeps)
+    # size one step (a bounded sample of the `full`-sweep step) to ~2 s of CPU work
+    coef = oracle.coefficients(w.F, w.rho_l, w.rho_g, w.dx, w.dy, w.dz)
+    p = np.zeros_like(w.rhs)
+    t0 = time.perf_counter()
+    oracle.sweep(coef, w.rhs, p, w.omega, 1)
+    per = time.perf_counter() - t0
+    n = max(1, min(full, int(2.0 / max(per, 1e-6))))
+
+    def step():
+        c = oracle.coefficients(w.F, w.rho_l, w.rho_g, w.dx, w.dy, w.dz)
+        q = np.zeros_like(w.rhs)
+        oracle.sweep(c, w.rhs, q, w.omega, n)
+        return oracle.residual(c, w.rhs, q)
+
+    for _ in range(args.warmup):
+        step()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step()
+    dt = time.perf_counter() - t0
+    value = w.cells * n * args.steps / dt / 1e9
+    sample = f"{w.name}: each step = coefficient build + {n} of {full} sweeps + residual"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": w.name, "cells": w.cells, "sweeps_per_step": n,
+                   "note": "CPU oracle (oracle/ps_oracle.c) on host cores; the paper has no code"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.threads(), "kind": "oracle",
+                         "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+# --------------------------------------------------------------------------- our arm
+def run_ours(args, rank):
+    import torch
+    from paper_2104_01636_b200 import binding, build, replicas, workload as wl
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the CUDA path is the only path)")
+    torch.cuda.set_device(rank.local_rank)
+    build.build()
+    binding.load()
+    w = wl.make_config(args.config, seed_offset=replicas.seed_offset(rank))
+    sweeps = sweeps_for(args.config, args.sweeps)
+    shape = (w.nz, w.ny, w.nx)
+    kernel = {"auto": binding.KERNEL_AUTO, "twopass": binding.KERNEL_TWOPASS,
+              "fused": binding.KERNEL_FUSED, "fused_t2": binding.KERNEL_FUSED_T2}[args.kernel]
+
+    F_h = torch.from_numpy(w.F).pin_memory()
+    rhs_h = torch.from_numpy(w.rhs).pin_memory()
+    p_h = torch.zeros(shape, dtype=torch.float64).pin_memory()
+    F_d, rhs_d = F_h.cuda(), rhs_h.cuda()
+    p_d = torch.zeros_like(rhs_d)
+
+    s = binding.PoissonSolver(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz)
+    s.set_kernel(kernel)
+    kname = binding.KERNEL_NAMES[s.get_kernel()]
+
+    def step():
+        p_d.zero_()
+        s.set_fraction(F_d, w.rho_l, w.rho_g)
+        return s.solve(rhs_d, p_d, w.omega, sweeps, 0.0)
+
+    for _ in range(args.warmup):
+        info = step()
+    s.enable_timing(True)
+    s.timing()
+    clocks = ClockSampler(rank.local_rank)
+    if rank.rank == 0:
+        clocks.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    replicas.barrier(rank)
+    torch.cuda.synchronize()
+    l0 = s.launch_count()
+    ev0.record()
+    for _ in range(args.steps):
+        info = step()
+    ev1.record()
+    torch.cuda.synchronize()
+    replicas.barrier(rank)
+    launches = s.launch_count() - l0
+    secs = ev0.elapsed_time(ev1) / 1e3
+    sweep_ms, sweep_launches = s.timing()
+    s.enable_timing(False)
+    clk = clocks.stop() if rank.rank == 0 else None
+    value, units, tmax = replicas.aggregate_throughput(rank, float(w.cells) * sweeps * args.steps,
+                                                       secs)
+
+    # ---- end to end: host buffers, copies inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        def step_host():
+            p_h.zero_()
+            return s.solve_host(F_h, w.rho_l, w.rho_g, rhs_h, p_h, w.omega, sweeps, 0.0)
+        step_host()
+        replicas.barrier(rank)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        ev0.record()
+        for _ in range(args.steps):
+            step_host()
+        ev1.record()
+        torch.cuda.synchronize()
+        t_host = time.perf_counter() - t0
+        replicas.barrier(rank)
+        secs_e = max(ev0.elapsed_time(ev1) / 1e3, t_host)   # pageable-style sync copies: wall clock
+        v_e, _, _ = replicas.aggregate_throughput(rank, float(w.cells) * sweeps * args.steps,
+                                                  secs_e)
+        e2e = {"value": v_e / 1e9, "unit": UNIT, "h2d_bytes_per_step": 3 * 8 * w.cells,
+               "d2h_bytes_per_step": 8 * w.cells + 24, "ms_per_step": 1e3 * secs_e / args.steps}
+
+    if rank.rank != 0:
+        return
+    peak, peak_src = measured_peak()
+    launch_s = sweep_ms / 1e3 / max(sweep_launches, 1)
+    algo_bytes = ALGO_BYTES_PER_CELL_LAUNCH[kname] * w.cells
+    achieved = algo_bytes / launch_s / 1e9
+    line = {
+        "metric": METRIC, "value": value / 1e9, "unit": UNIT, "n_gpus": rank.world,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tmax / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": w.name, "cells": w.cells, "sweeps_per_step": sweeps,
+                   "omega": w.omega, "kernel": kname, "spheres": int(len(w.centres)),
+                   "step": "ps_set_fraction + ps_solve(sweeps, tol=0) incl. residual",
+                   "l2": "working set 1.3 GB+ >> 126 MB L2 (no flush needed)" if w.cells > 8e6
+                         else "L2-resident working set (not an HBM measurement)",
+                   "parallelism": "replicas" if rank.world > 1 else "single GPU"},
+        "final_res_rel": info.res_rel,
+        "sweep_only_gcells_per_s": w.cells * (sweep_launches * (0.5 if kname == "twopass" else
+                                              2.0 if kname == "fused_t2" else 1.0))
+                                   / (sweep_ms / 1e3) / 1e9 if sweep_ms > 0 else None,
+        "gpu_launches": launches,
+        "clocks": clk,
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                     "frac": achieved / peak, "traffic": ncu_traffic(kname, args.config),
+                     "kernel": kname, "algorithmic_bytes_per_launch": algo_bytes,
+                     "avg_launch_ms": 1e3 * launch_s, "launches_timed": sweep_launches,
+                     "peak_source": peak_src},
+    }
+    if e2e:
+        line["e2e"] = e2e
+    if rank.world == 1 and not args.no_cpu_baseline:
+        line["cpu_baseline"] = oracle_sample(w, args.cpu_seconds)
+    print(json.dumps(line))
+
+
+def main():
+    args = parse_args()
+    from paper_2104_01636_b200 import replicas
+    if args.impl == "reference":       # rank 0 alone runs it; no process group is needed
+        run_reference(args, replicas.Rank(int(os.environ.get("RANK", "0")),
+                                          int(os.environ.get("LOCAL_RANK", "0")),
+                                          int(os.environ.get("WORLD_SIZE", "1")), None))
+        return
+    rank = replicas.init()
+    try:
+        run_ours(args, rank)
+    finally:
+        replicas.finalize(rank)
+
+
+if __name__ == "__main__":
+    main()

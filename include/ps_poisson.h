@@ -1,0 +1,152 @@
+/*
+ * ps_poisson.h -- C ABI of libps_poisson.so: B200 (sm_100a) red-black SOR solver for the
+ * variable-coefficient pressure Poisson equation of the projection step of Kumar & Vanka
+ * (arXiv 2104.01636):
+ *
+ *        div( grad p / rho )^{n+1} = rhs                       PAPER.md:109-111 (§2.2 step 11)
+ *        rho = alpha rho_l + (1 - alpha) rho_g                 PAPER.md:66 eq (4), :92 step 4
+ *        face values by linear averaging c->f (rho_f)
+ *        no-penetration walls in x and y, periodic z
+ *        uniform Cartesian collocated grid
+ *        "red black SOR relaxation scheme ... on a GPU"
+ *
+ * Everything the paper leaves open (omega, colour order, norm, stopping rule, wall treatment of
+ * p) follows DESIGN.md "Readings" S1-S10.
+ *
+ * Conventions
+ *   Grid nx x ny x nz, cell (i,j,k), linear index n = i + nx*(j + ny*k): x fastest, z slowest.
+ *   All fields are fp64.  F is the LIQUID volume fraction (alpha of the paper).
+ *   Discrete operator (A p)_c = sum_f a_f (p_nb - p_c), a_f = (1/h_f^2) / (0.5 (rho_c + rho_nb)),
+ *   a_f = 0 on the x and y walls, z faces wrap.  One "sweep" = red half-sweep ((i+j+k) even)
+ *   followed by black half-sweep = N cell updates:
+ *        g = (sum_f a_f p_nb - rhs_c) / sum_f a_f ;   p_c <- p_c + omega (g - p_c).
+ *
+ * Pointers
+ *   *_dev  : device memory owned by the caller (e.g. a torch tensor), contiguous natural layout,
+ *            16-byte aligned, nx*ny*nz doubles.  Never freed or retained past the call.
+ *   *_host : host memory owned by the caller (pageable or pinned), same layout.
+ *   Output scalars / ps_info are host pointers.
+ *
+ * Errors: every entry point returns 0 (PS_OK) or a negative code; nothing throws, aborts or
+ * prints.  There is NO CPU fallback: without a CUDA device every compute call returns PS_ECUDA.
+ * A ps_ctx is not thread-safe; distinct contexts are independent.
+ */
+#ifndef PS_POISSON_H
+#define PS_POISSON_H
+#include <stddef.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PS_OK       0
+#define PS_EINVAL  (-1)   /* bad argument (see each call)                                  */
+#define PS_ESTATE  (-2)   /* call order: solve/residual/sweeps before ps_set_fraction      */
+#define PS_ECUDA   (-3)   /* a CUDA runtime call failed; ps_strerror gives the CUDA string */
+#define PS_ENOMEM  (-4)   /* host or device allocation failed                              */
+
+/* Sweep kernel variants (ps_set_kernel).  All give bitwise identical p. */
+#define PS_KERNEL_AUTO     0   /* fastest variant the grid shape allows                     */
+#define PS_KERNEL_TWOPASS  1   /* generic: one launch per colour, in place, any nx,ny>=1    */
+#define PS_KERNEL_FUSED    2   /* red+black fused in one z-marching pass, ping-pong p       */
+#define PS_KERNEL_FUSED_T2 3   /* two fused sweeps temporally blocked per launch            */
+
+typedef struct ps_ctx ps_ctx;   /* opaque; one per grid */
+
+typedef struct {
+    int    sweeps;      /* sweeps performed by this call                                   */
+    int    converged;   /* 1: tol > 0 and res_rel <= tol at the last check; else 0         */
+    double res_abs;     /* || rhs - A p ||_2  (plain Euclidean, no 1/N)                    */
+    double res_rel;     /* res_abs / ||rhs||_2   (res_abs itself if ||rhs||_2 == 0)        */
+    double rhs_norm;    /* || rhs ||_2                                                     */
+} ps_info;
+
+/* Create a solver for an nx x ny x nz grid with spacings dx,dy,dz on the current CUDA device.
+ * PS_EINVAL: out NULL; nx,ny < 1; nz < 2 or nz odd (the red-black colouring must stay
+ * consistent across the periodic wrap); dx,dy,dz not finite or <= 0.
+ * Allocates its own workspace (ps_workspace_bytes) with cudaMalloc unless ps_set_workspace
+ * supplies one before the first ps_set_fraction. */
+int ps_create(ps_ctx **out, int nx, int ny, int nz, double dx, double dy, double dz);
+
+/* Free the context and any workspace the library allocated itself.  NULL is allowed. */
+int ps_destroy(ps_ctx *c);
+
+/* Bytes of device workspace the context needs: face coefficients ax, ay, az, the second p
+ * buffer of the fused kernels, reduction partials and device scalars. */
+size_t ps_workspace_bytes(const ps_ctx *c);
+
+/* Hand the context a caller-owned device workspace (256-byte aligned, >= ps_workspace_bytes).
+ * It is retained until ps_destroy or the next ps_set_workspace; coefficients built before the
+ * switch are lost (ps_set_fraction must be called again).  PS_EINVAL if too small/misaligned. */
+int ps_set_workspace(ps_ctx *c, void *ws_dev, size_t bytes);
+
+/* CUDA stream (a cudaStream_t passed as void*) on which every later call enqueues its work.
+ * Default: the legacy default stream (NULL). */
+int ps_set_stream(ps_ctx *c, void *cuda_stream);
+
+/* Residual check cadence K of ps_solve (default 50, K >= 1). */
+int ps_set_check_interval(ps_ctx *c, int K);
+
+/* Choose the sweep kernel (PS_KERNEL_*).  PS_EINVAL if the grid shape does not allow the
+ * variant (the fused kernels need nx % 4 == 0, nx >= 8, ny >= 4, nz >= 4). */
+int ps_set_kernel(ps_ctx *c, int variant);
+int ps_get_kernel(const ps_ctx *c);          /* the variant AUTO resolved to, or the one set */
+
+/* Step 4 of the paper's time step + face coefficients:
+ * rho = rho_l F + rho_g (1-F); ax,ay,az = (1/h^2)/(0.5 (rho_c + rho_nb)) for the +x,+y,+z
+ * face of every cell, 0 on the +x / +y wall faces, +z wraps.  One launch, asynchronous on
+ * the stream.  F_dev is only read during the call.  PS_EINVAL: NULL, rho_l or rho_g <= 0 or
+ * not finite.  Not checked on the device: F in [0,1], finite. */
+int ps_set_fraction(ps_ctx *c, const double *F_dev, double rho_l, double rho_g);
+
+/* Copy the face coefficients out in natural layout (device pointers, any may be NULL). */
+int ps_export_coefficients(ps_ctx *c, double *ax_dev, double *ay_dev, double *az_dev);
+
+/* Red-black SOR on A p = rhs starting from the caller's p (in/out).
+ *   for s = 1..max_sweeps { red; black; if (tol > 0 && (s % K == 0 || s == max_sweeps)) check }
+ * stopping at the first check with ||r||_2/||rhs||_2 <= tol.  tol <= 0: exactly max_sweeps
+ * sweeps, norm computed once at the end.  Synchronises the stream before returning; the only
+ * device->host traffic are the 16-byte norm read-backs.  Hitting max_sweeps is not an error
+ * (info->converged = 0).  info may be NULL.
+ * PS_EINVAL: NULL rhs/p, omega not in (0,2), max_sweeps < 0.  PS_ESTATE: no coefficients. */
+int ps_solve(ps_ctx *c, const double *rhs_dev, double *p_dev, double omega, int max_sweeps,
+             double tol, ps_info *info);
+
+/* Exactly n sweeps, enqueued asynchronously: no norm, no host synchronisation (the throughput
+ * window of bench.py; time it with events on the stream). */
+int ps_sweeps(ps_ctx *c, const double *rhs_dev, double *p_dev, double omega, int n);
+
+/* One colour only (colour 0 = red = (i+j+k) even, 1 = black), in place, generic kernel;
+ * asynchronous.  For parity tests of the half-sweep itself. */
+int ps_half_sweep(ps_ctx *c, const double *rhs_dev, double *p_dev, double omega, int colour);
+
+/* ||rhs - A p||_2 and its ratio to ||rhs||_2 by the deterministic two-pass reduction
+ * (fixed partition, warp-shuffle tree, single-block fixed-order final pass; no atomics).
+ * Synchronises the stream.  Outputs are host pointers; res_rel / rhs_norm may be NULL. */
+int ps_residual(ps_ctx *c, const double *rhs_dev, const double *p_dev, double *res_abs,
+                double *res_rel, double *rhs_norm);
+
+/* The whole path on HOST buffers (the end-to-end leg of bench.py): H2D of F and rhs and p,
+ * ps_set_fraction, ps_solve, D2H of p.  Staging buffers live in the context and are allocated
+ * on first use.  Same errors as the calls it wraps. */
+int ps_solve_host(ps_ctx *c, const double *F_host, double rho_l, double rho_g,
+                  const double *rhs_host, double *p_host, double omega, int max_sweeps,
+                  double tol, ps_info *info);
+
+/* Device-side timing of the sweep kernels, for the roofline line of bench.py.  When enabled,
+ * every batch of sweep launches issued by ps_solve / ps_sweeps / ps_solve_host is bracketed by a
+ * pair of CUDA events on the context's stream.  ps_timing synchronises the stream, adds up the
+ * elapsed times since the last ps_timing call and returns them with the number of sweep-kernel
+ * launches they cover (sweep_ms / launches = average launch duration); either may be NULL. */
+int ps_enable_timing(ps_ctx *c, int on);
+int ps_timing(ps_ctx *c, double *sweep_ms, long long *sweep_launches);
+
+/* Kernels launched by this context since ps_create (bench.py's gpu_launches). */
+long long ps_launch_count(const ps_ctx *c);
+
+/* Text for a return code; for PS_ECUDA the last CUDA error string seen by this thread. */
+const char *ps_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

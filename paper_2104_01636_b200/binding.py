@@ -1,0 +1,235 @@
+"""Thin ctypes binding of include/ps_poisson.h -- argument marshalling only.
+
+Every step of the path (coefficient build, sweeps, residual, norms) runs in the CUDA kernels
+behind libps_poisson.so.  PyTorch is used for device memory and streams: arguments are CUDA
+float64 tensors of shape (nz, ny, nx) (linear index n = i + nx*(j + ny*k)), handed over as raw
+device pointers; the library enqueues on torch's current stream.
+
+There is no CPU fallback: if the library is not built, `load()` raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from dataclasses import dataclass
+
+from . import build as _build
+
+PS_OK, PS_EINVAL, PS_ESTATE, PS_ECUDA, PS_ENOMEM = 0, -1, -2, -3, -4
+KERNEL_AUTO, KERNEL_TWOPASS, KERNEL_FUSED, KERNEL_FUSED_T2 = 0, 1, 2, 3
+KERNEL_NAMES = {KERNEL_AUTO: "auto", KERNEL_TWOPASS: "twopass", KERNEL_FUSED: "fused",
+                KERNEL_FUSED_T2: "fused_t2"}
+
+# every symbol include/ps_poisson.h declares (tests check the library exports each one)
+SYMBOLS = ("ps_create", "ps_destroy", "ps_workspace_bytes", "ps_set_workspace", "ps_set_stream",
+           "ps_set_check_interval", "ps_set_kernel", "ps_get_kernel", "ps_set_fraction",
+           "ps_export_coefficients", "ps_solve", "ps_sweeps", "ps_half_sweep", "ps_residual",
+           "ps_solve_host", "ps_enable_timing", "ps_timing", "ps_launch_count", "ps_strerror")
+
+
+class PsError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"libps_poisson: {msg} (code {code})")
+        self.code = code
+
+
+class _Info(ctypes.Structure):
+    _fields_ = [("sweeps", ctypes.c_int), ("converged", ctypes.c_int),
+                ("res_abs", ctypes.c_double), ("res_rel", ctypes.c_double),
+                ("rhs_norm", ctypes.c_double)]
+
+
+@dataclass
+class Info:
+    sweeps: int
+    converged: bool
+    res_abs: float
+    res_rel: float
+    rhs_norm: float
+
+
+_lib = None
+
+
+def load(path: str | None = None) -> ctypes.CDLL:
+    """dlopen libps_poisson.so and declare the prototypes.  Raises if it is not built."""
+    global _lib
+    if _lib is not None and path is None:
+        return _lib
+    path = path or _build.LIB
+    if not os.path.exists(path):
+        raise RuntimeError(f"{path} is missing: run `python -m paper_2104_01636_b200.build` "
+                           "(the CUDA extension is the only compute path; there is no fallback)")
+    lib = ctypes.CDLL(path)
+    vp, i, d, dp = ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.POINTER(ctypes.c_double)
+    lib.ps_create.argtypes = [ctypes.POINTER(vp), i, i, i, d, d, d]
+    lib.ps_destroy.argtypes = [vp]
+    lib.ps_workspace_bytes.argtypes = [vp]
+    lib.ps_workspace_bytes.restype = ctypes.c_size_t
+    lib.ps_set_workspace.argtypes = [vp, vp, ctypes.c_size_t]
+    lib.ps_set_stream.argtypes = [vp, vp]
+    lib.ps_set_check_interval.argtypes = [vp, i]
+    lib.ps_set_kernel.argtypes = [vp, i]
+    lib.ps_get_kernel.argtypes = [vp]
+    lib.ps_set_fraction.argtypes = [vp, vp, d, d]
+    lib.ps_export_coefficients.argtypes = [vp, vp, vp, vp]
+    lib.ps_solve.argtypes = [vp, vp, vp, d, i, d, ctypes.POINTER(_Info)]
+    lib.ps_sweeps.argtypes = [vp, vp, vp, d, i]
+    lib.ps_half_sweep.argtypes = [vp, vp, vp, d, i]
+    lib.ps_residual.argtypes = [vp, vp, vp, dp, dp, dp]
+    lib.ps_solve_host.argtypes = [vp, vp, d, d, vp, vp, d, i, d, ctypes.POINTER(_Info)]
+    lib.ps_enable_timing.argtypes = [vp, i]
+    lib.ps_timing.argtypes = [vp, dp, ctypes.POINTER(ctypes.c_longlong)]
+    lib.ps_launch_count.argtypes = [vp]
+    lib.ps_launch_count.restype = ctypes.c_longlong
+    lib.ps_strerror.argtypes = [i]
+    lib.ps_strerror.restype = ctypes.c_char_p
+    if path == _build.LIB:
+        _lib = lib
+    return lib
+
+
+def _check(lib, rc: int):
+    if rc != PS_OK:
+        raise PsError(rc, lib.ps_strerror(rc).decode())
+
+
+def _dev_ptr(t, shape, name):
+    import torch
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64
+            and t.is_contiguous() and tuple(t.shape) == tuple(shape)):
+        raise TypeError(f"{name}: expected a contiguous CUDA float64 tensor of shape {tuple(shape)}")
+    return ctypes.c_void_p(t.data_ptr())
+
+
+def _host_ptr(a, shape, name):
+    import numpy as np
+    import torch
+    if isinstance(a, torch.Tensor):
+        if a.is_cuda or a.dtype != torch.float64 or not a.is_contiguous() or tuple(a.shape) != tuple(shape):
+            raise TypeError(f"{name}: expected a contiguous host float64 tensor of shape {tuple(shape)}")
+        return ctypes.c_void_p(a.data_ptr())
+    if not (isinstance(a, np.ndarray) and a.dtype == np.float64 and a.flags["C_CONTIGUOUS"]
+            and tuple(a.shape) == tuple(shape)):
+        raise TypeError(f"{name}: expected a C-contiguous float64 array of shape {tuple(shape)}")
+    return ctypes.c_void_p(a.ctypes.data)
+
+
+class PoissonSolver:
+    """ps_create / ps_set_fraction / ps_solve / ps_residual with the names of the C ABI."""
+
+    def __init__(self, nx: int, ny: int, nz: int, dx: float, dy: float, dz: float,
+                 workspace: bool = True):
+        import torch
+        self._lib = load()
+        self._h = ctypes.c_void_p()
+        self.nx, self.ny, self.nz = nx, ny, nz
+        self.shape = (nz, ny, nx)
+        _check(self._lib, self._lib.ps_create(ctypes.byref(self._h), nx, ny, nz, dx, dy, dz))
+        self._ws = None
+        if workspace:      # torch owns the device memory (north_star: "PyTorch ... device memory")
+            nbytes = self._lib.ps_workspace_bytes(self._h)
+            self._ws = torch.empty(nbytes + 256, dtype=torch.uint8, device="cuda")
+            base = (self._ws.data_ptr() + 255) // 256 * 256
+            _check(self._lib, self._lib.ps_set_workspace(self._h, ctypes.c_void_p(base), nbytes))
+
+    # -- lifetime
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            self._lib.ps_destroy(self._h)
+            self._h = ctypes.c_void_p()
+        self._ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def _sync_stream(self):
+        import torch
+        s = torch.cuda.current_stream().cuda_stream
+        _check(self._lib, self._lib.ps_set_stream(self._h, ctypes.c_void_p(s)))
+
+    # -- options
+    def set_check_interval(self, K: int):
+        _check(self._lib, self._lib.ps_set_check_interval(self._h, K))
+
+    def set_kernel(self, variant: int):
+        _check(self._lib, self._lib.ps_set_kernel(self._h, variant))
+
+    def get_kernel(self) -> int:
+        return self._lib.ps_get_kernel(self._h)
+
+    def workspace_bytes(self) -> int:
+        return self._lib.ps_workspace_bytes(self._h)
+
+    def enable_timing(self, on: bool = True):
+        _check(self._lib, self._lib.ps_enable_timing(self._h, int(on)))
+
+    def timing(self):
+        """(sweep_ms, sweep_launches) accumulated since the last call; synchronises the stream."""
+        ms, n = ctypes.c_double(), ctypes.c_longlong()
+        _check(self._lib, self._lib.ps_timing(self._h, ctypes.byref(ms), ctypes.byref(n)))
+        return ms.value, n.value
+
+    def launch_count(self) -> int:
+        return self._lib.ps_launch_count(self._h)
+
+    # -- the path
+    def set_fraction(self, F, rho_l: float, rho_g: float):
+        self._sync_stream()
+        _check(self._lib, self._lib.ps_set_fraction(self._h, _dev_ptr(F, self.shape, "F"),
+                                                    rho_l, rho_g))
+
+    def export_coefficients(self):
+        import torch
+        self._sync_stream()
+        out = [torch.empty(self.shape, dtype=torch.float64, device="cuda") for _ in range(3)]
+        _check(self._lib, self._lib.ps_export_coefficients(
+            self._h, *[ctypes.c_void_p(t.data_ptr()) for t in out]))
+        return tuple(out)
+
+    def solve(self, rhs, p, omega: float, max_sweeps: int, tol: float) -> Info:
+        self._sync_stream()
+        info = _Info()
+        _check(self._lib, self._lib.ps_solve(self._h, _dev_ptr(rhs, self.shape, "rhs"),
+                                             _dev_ptr(p, self.shape, "p"), omega, max_sweeps,
+                                             tol, ctypes.byref(info)))
+        return Info(info.sweeps, bool(info.converged), info.res_abs, info.res_rel, info.rhs_norm)
+
+    def sweeps(self, rhs, p, omega: float, n: int):
+        self._sync_stream()
+        _check(self._lib, self._lib.ps_sweeps(self._h, _dev_ptr(rhs, self.shape, "rhs"),
+                                              _dev_ptr(p, self.shape, "p"), omega, n))
+
+    def half_sweep(self, rhs, p, omega: float, colour: int):
+        self._sync_stream()
+        _check(self._lib, self._lib.ps_half_sweep(self._h, _dev_ptr(rhs, self.shape, "rhs"),
+                                                  _dev_ptr(p, self.shape, "p"), omega, colour))
+
+    def residual(self, rhs, p):
+        """(res_abs, res_rel, rhs_norm)"""
+        self._sync_stream()
+        ra, rr, bn = ctypes.c_double(), ctypes.c_double(), ctypes.c_double()
+        _check(self._lib, self._lib.ps_residual(self._h, _dev_ptr(rhs, self.shape, "rhs"),
+                                                _dev_ptr(p, self.shape, "p"), ctypes.byref(ra),
+                                                ctypes.byref(rr), ctypes.byref(bn)))
+        return ra.value, rr.value, bn.value
+
+    def solve_host(self, F, rho_l: float, rho_g: float, rhs, p, omega: float, max_sweeps: int,
+                   tol: float) -> Info:
+        """Whole path on HOST arrays (numpy or CPU torch tensors); p is updated in place."""
+        self._sync_stream()
+        info = _Info()
+        _check(self._lib, self._lib.ps_solve_host(
+            self._h, _host_ptr(F, self.shape, "F"), rho_l, rho_g,
+            _host_ptr(rhs, self.shape, "rhs"), _host_ptr(p, self.shape, "p"), omega, max_sweeps,
+            tol, ctypes.byref(info)))
+        return Info(info.sweeps, bool(info.converged), info.res_abs, info.res_rel, info.rhs_norm)

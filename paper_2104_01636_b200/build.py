@@ -1,0 +1,67 @@
+"""Compile the CUDA path into paper_2104_01636_b200/libps_poisson.so (in-tree, sm_100a only).
+
+    python -m paper_2104_01636_b200.build [--force]
+
+nvcc cross-compiles without a GPU.  Flags that matter for parity:
+`--fmad=false` (no FMA contraction: every product and sum of the SOR update rounds separately,
+as in the oracle's `-ffp-contract=off`), never `-use_fast_math`; fp64 division and sqrt are
+IEEE-correct regardless.
+"""
+from __future__ import annotations
+
+import os
+import shutil
+import subprocess
+import sys
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_CSRC = os.path.join(_HERE, "csrc")
+_INC = os.path.join(os.path.dirname(_HERE), "include")
+LIB = os.path.join(_HERE, "libps_poisson.so")
+SOURCES = ["ps_api.cu"]
+HEADERS = ["ps_kernels_generic.cuh", "ps_kernels_fused.cuh"]
+
+NVCC_FLAGS = [
+    "-gencode", "arch=compute_100a,code=sm_100a",
+    "-std=c++17", "-O3", "--fmad=false", "-lineinfo",
+    "-Xcompiler", "-fPIC", "-shared", "-cudart", "static",
+]
+
+
+def _nvcc() -> str:
+    for cand in (os.environ.get("NVCC"), shutil.which("nvcc"), "/usr/local/cuda/bin/nvcc"):
+        if cand and os.path.exists(cand):
+            return cand
+    raise RuntimeError("nvcc not found: the CUDA path cannot be built (there is no CPU fallback)")
+
+
+def _deps():
+    yield os.path.join(_INC, "ps_poisson.h")
+    for f in SOURCES + HEADERS:
+        yield os.path.join(_CSRC, f)
+
+
+def up_to_date() -> bool:
+    return os.path.exists(LIB) and os.path.getmtime(LIB) >= max(os.path.getmtime(d) for d in _deps())
+
+
+def build(force: bool = False, verbose: bool = False) -> str:
+    """Build libps_poisson.so if missing or older than its sources; returns its path."""
+    if not force and up_to_date():
+        return LIB
+    tmp = f"{LIB}.{os.getpid()}.tmp"
+    cmd = [_nvcc(), *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []),
+           "-o", tmp, *[os.path.join(_CSRC, s) for s in SOURCES]]
+    res = subprocess.run(cmd, cwd=_CSRC, capture_output=True, text=True)
+    if res.returncode != 0:
+        if os.path.exists(tmp):
+            os.remove(tmp)
+        raise RuntimeError("nvcc failed:\n" + " ".join(cmd) + "\n" + res.stdout + res.stderr)
+    if verbose:
+        sys.stderr.write(res.stdout + res.stderr)
+    os.replace(tmp, LIB)
+    return LIB
+
+
+if __name__ == "__main__":
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

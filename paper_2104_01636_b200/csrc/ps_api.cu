@@ -1,0 +1,459 @@
+// ps_api.cu -- the C ABI of include/ps_poisson.h: context, workspace, launch logic.
+// Every step of the path runs in the CUDA kernels of ps_kernels_*.cuh; this file only validates
+// arguments, carves the workspace and enqueues launches.  There is no CPU fallback.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/ps_poisson.h"
+#include "ps_kernels_generic.cuh"
+#include "ps_kernels_fused.cuh"
+
+namespace {
+
+thread_local char g_cuda_msg[256] = "no CUDA error recorded";
+
+int cuda_fail(cudaError_t e)
+{
+    snprintf(g_cuda_msg, sizeof g_cuda_msg, "CUDA error %d: %s", (int)e, cudaGetErrorString(e));
+    return PS_ECUDA;
+}
+
+#define PS_CUDA(call)                                   \
+    do {                                                \
+        cudaError_t e_ = (call);                        \
+        if (e_ != cudaSuccess) return cuda_fail(e_);    \
+    } while (0)
+
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+}  // namespace
+
+struct ps_ctx {
+    ps::Grid g;
+    double dx, dy, dz;
+    cudaStream_t stream;
+    int K;                 // residual check cadence
+    int variant_req;       // what the caller asked for (PS_KERNEL_*)
+    int variant;           // resolved
+    bool have_coef;
+    int sm_count;
+    long long launches;
+    // workspace
+    void *ws;
+    size_t ws_bytes;
+    bool ws_owned;
+    double *ax, *ay, *az, *p_alt, *partR2, *partB2, *scal;   // scal: 3 doubles out
+    int *done;
+    int nparts;
+    double *h_scal;        // pinned, 4 doubles
+    // staging of ps_solve_host
+    double *st_F, *st_rhs, *st_p;
+    ps::FusedPlan fused;
+    // optional event timing of the sweep launches (ps_enable_timing)
+    bool timing;
+    std::vector<cudaEvent_t> *ev;      // pairs: start, stop
+    size_t ev_used;
+    long long timed_launches;
+};
+
+namespace {
+
+size_t field_bytes(const ps_ctx *c) { return align_up(c->g.cells() * sizeof(double), 256); }
+
+size_t workspace_bytes(const ps_ctx *c)
+{
+    return 4 * field_bytes(c) + 2 * align_up((size_t)c->nparts * sizeof(double), 256) + 256 + 256;
+}
+
+void carve(ps_ctx *c, void *base)
+{
+    char *q = (char *)base;
+    const size_t fb = field_bytes(c), pb = align_up((size_t)c->nparts * sizeof(double), 256);
+    c->ax = (double *)q; q += fb;
+    c->ay = (double *)q; q += fb;
+    c->az = (double *)q; q += fb;
+    c->p_alt = (double *)q; q += fb;
+    c->partR2 = (double *)q; q += pb;
+    c->partB2 = (double *)q; q += pb;
+    c->scal = (double *)q; q += 256;
+    c->done = (int *)q;
+}
+
+int ensure_workspace(ps_ctx *c)
+{
+    if (c->ws) return PS_OK;
+    void *w = nullptr;
+    cudaError_t e = cudaMalloc(&w, workspace_bytes(c));
+    if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); return PS_ENOMEM; }
+    if (e != cudaSuccess) return cuda_fail(e);
+    c->ws = w;
+    c->ws_bytes = workspace_bytes(c);
+    c->ws_owned = true;
+    carve(c, w);
+    return PS_OK;
+}
+
+int resolve_variant(const ps_ctx *c, int req)
+{
+    const bool fused_ok = ps::fused_shape_ok(c->g);
+    if (req == PS_KERNEL_AUTO) return fused_ok ? PS_KERNEL_FUSED : PS_KERNEL_TWOPASS;
+    if ((req == PS_KERNEL_FUSED || req == PS_KERNEL_FUSED_T2) && !fused_ok) return -1;
+    if (req < PS_KERNEL_AUTO || req > PS_KERNEL_FUSED_T2) return -1;
+    return req;
+}
+
+int grid_for(const ps_ctx *c, size_t work_items, int threads)
+{
+    // enough blocks to cover the work once, capped at 32 resident waves of the device
+    size_t blocks = (work_items + threads - 1) / threads;
+    const size_t cap = (size_t)c->sm_count * 8 * 32;
+    if (blocks > cap) blocks = cap;
+    if (blocks < 1) blocks = 1;
+    return (int)blocks;
+}
+
+int launch_half_sweep(ps_ctx *c, const double *rhs, double *p, double omega, int colour)
+{
+    const size_t items = (size_t)((c->g.nx + 1) / 2) * c->g.ny * c->g.nz;
+    ps::ps_half_sweep_kernel<<<grid_for(c, items, 256), 256, 0, c->stream>>>(
+        c->g, c->ax, c->ay, c->az, rhs, p, omega, colour);
+    c->launches++;
+    PS_CUDA(cudaGetLastError());
+    return PS_OK;
+}
+
+// n sweeps on p (in/out), any variant.  The fused variants ping-pong between p and p_alt and
+// leave the result in p (an odd count ends with one device-to-device copy).
+int run_sweeps_untimed(ps_ctx *c, const double *rhs, double *p, double omega, int n);
+
+int run_sweeps(ps_ctx *c, const double *rhs, double *p, double omega, int n)
+{
+    if (n <= 0) return PS_OK;
+    if (!c->timing) return run_sweeps_untimed(c, rhs, p, omega, n);
+    if (c->ev_used + 2 > c->ev->size()) {
+        cudaEvent_t a, b;
+        PS_CUDA(cudaEventCreate(&a));
+        PS_CUDA(cudaEventCreate(&b));
+        c->ev->push_back(a);
+        c->ev->push_back(b);
+    }
+    const long long before = c->launches;
+    PS_CUDA(cudaEventRecord((*c->ev)[c->ev_used], c->stream));
+    const int rc = run_sweeps_untimed(c, rhs, p, omega, n);
+    PS_CUDA(cudaEventRecord((*c->ev)[c->ev_used + 1], c->stream));
+    c->ev_used += 2;
+    c->timed_launches += c->launches - before;
+    return rc;
+}
+
+int run_sweeps_untimed(ps_ctx *c, const double *rhs, double *p, double omega, int n)
+{
+    if (c->variant == PS_KERNEL_TWOPASS) {
+        for (int s = 0; s < n; ++s) {
+            int rc = launch_half_sweep(c, rhs, p, omega, 0);
+            if (rc) return rc;
+            rc = launch_half_sweep(c, rhs, p, omega, 1);
+            if (rc) return rc;
+        }
+        return PS_OK;
+    }
+    double *src = p, *dst = c->p_alt;
+    int left = n;
+    while (left > 0) {
+        int did = 0;
+        cudaError_t e = ps::launch_fused(c->fused, c->g, c->ax, c->ay, c->az, rhs, src, dst, omega,
+                                         (c->variant == PS_KERNEL_FUSED_T2 && left >= 2) ? 2 : 1,
+                                         c->stream, &did);
+        c->launches++;
+        if (e != cudaSuccess) return cuda_fail(e);
+        left -= did;
+        double *t = src; src = dst; dst = t;
+    }
+    if (src != p) {
+        PS_CUDA(cudaMemcpyAsync(p, src, c->g.cells() * sizeof(double), cudaMemcpyDeviceToDevice,
+                                c->stream));
+    }
+    return PS_OK;
+}
+
+int enqueue_residual(ps_ctx *c, const double *rhs, const double *p, double tol)
+{
+    ps::ps_residual_partial_kernel<<<c->nparts, ps::RED_THREADS, 0, c->stream>>>(
+        c->g, c->ax, c->ay, c->az, rhs, p, c->partR2, c->partB2);
+    c->launches++;
+    PS_CUDA(cudaGetLastError());
+    ps::ps_reduce_final_kernel<<<1, ps::FIN_THREADS, 0, c->stream>>>(c->partR2, c->partB2,
+                                                                    c->nparts, tol, c->scal,
+                                                                    nullptr);
+    c->launches++;
+    PS_CUDA(cudaGetLastError());
+    PS_CUDA(cudaMemcpyAsync(c->h_scal, c->scal, 3 * sizeof(double), cudaMemcpyDeviceToHost,
+                            c->stream));
+    return PS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int ps_create(ps_ctx **out, int nx, int ny, int nz, double dx, double dy, double dz)
+{
+    if (!out) return PS_EINVAL;
+    *out = nullptr;
+    if (nx < 1 || ny < 1 || nz < 2 || (nz & 1)) return PS_EINVAL;
+    if (!(dx > 0.0) || !(dy > 0.0) || !(dz > 0.0) || !std::isfinite(dx) || !std::isfinite(dy) ||
+        !std::isfinite(dz))
+        return PS_EINVAL;
+    if ((double)nx * (double)ny * (double)nz > 2.0e9) return PS_EINVAL;
+    int dev = 0, sms = 0;
+    PS_CUDA(cudaGetDevice(&dev));
+    PS_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    ps_ctx *c = new (std::nothrow) ps_ctx();
+    if (!c) return PS_ENOMEM;
+    c->g = ps::Grid{nx, ny, nz};
+    c->ev = new (std::nothrow) std::vector<cudaEvent_t>();
+    if (!c->ev) { delete c; return PS_ENOMEM; }
+    c->dx = dx; c->dy = dy; c->dz = dz;
+    c->K = 50;
+    c->sm_count = sms;
+    c->nparts = (int)((c->g.cells() + ps::RED_CHUNK - 1) / ps::RED_CHUNK);
+    c->variant_req = PS_KERNEL_AUTO;
+    c->variant = resolve_variant(c, PS_KERNEL_AUTO);
+    cudaError_t e = cudaMallocHost((void **)&c->h_scal, 4 * sizeof(double));
+    if (e != cudaSuccess) { delete c; return cuda_fail(e); }
+    e = ps::fused_plan_init(&c->fused, c->g, sms);
+    if (e != cudaSuccess) { cudaFreeHost(c->h_scal); delete c; return cuda_fail(e); }
+    *out = c;
+    return PS_OK;
+}
+
+int ps_destroy(ps_ctx *c)
+{
+    if (!c) return PS_OK;
+    if (c->ws && c->ws_owned) cudaFree(c->ws);
+    if (c->h_scal) cudaFreeHost(c->h_scal);
+    if (c->st_F) cudaFree(c->st_F);
+    if (c->st_rhs) cudaFree(c->st_rhs);
+    if (c->st_p) cudaFree(c->st_p);
+    if (c->ev) {
+        for (cudaEvent_t e : *c->ev) cudaEventDestroy(e);
+        delete c->ev;
+    }
+    delete c;
+    return PS_OK;
+}
+
+size_t ps_workspace_bytes(const ps_ctx *c) { return c ? workspace_bytes(c) : 0; }
+
+int ps_set_workspace(ps_ctx *c, void *ws_dev, size_t bytes)
+{
+    if (!c || !ws_dev) return PS_EINVAL;
+    if (((uintptr_t)ws_dev & 255u) != 0 || bytes < workspace_bytes(c)) return PS_EINVAL;
+    if (c->ws && c->ws_owned) cudaFree(c->ws);
+    c->ws = ws_dev;
+    c->ws_bytes = bytes;
+    c->ws_owned = false;
+    c->have_coef = false;
+    carve(c, ws_dev);
+    return PS_OK;
+}
+
+int ps_set_stream(ps_ctx *c, void *cuda_stream)
+{
+    if (!c) return PS_EINVAL;
+    c->stream = (cudaStream_t)cuda_stream;
+    return PS_OK;
+}
+
+int ps_set_check_interval(ps_ctx *c, int K)
+{
+    if (!c || K < 1) return PS_EINVAL;
+    c->K = K;
+    return PS_OK;
+}
+
+int ps_set_kernel(ps_ctx *c, int variant)
+{
+    if (!c) return PS_EINVAL;
+    const int v = resolve_variant(c, variant);
+    if (v < 0) return PS_EINVAL;
+    c->variant_req = variant;
+    c->variant = v;
+    return PS_OK;
+}
+
+int ps_get_kernel(const ps_ctx *c) { return c ? c->variant : PS_EINVAL; }
+
+int ps_set_fraction(ps_ctx *c, const double *F_dev, double rho_l, double rho_g)
+{
+    if (!c || !F_dev) return PS_EINVAL;
+    if (!(rho_l > 0.0) || !(rho_g > 0.0) || !std::isfinite(rho_l) || !std::isfinite(rho_g))
+        return PS_EINVAL;
+    int rc = ensure_workspace(c);
+    if (rc) return rc;
+    const double cx = 1.0 / (c->dx * c->dx), cy = 1.0 / (c->dy * c->dy), cz = 1.0 / (c->dz * c->dz);
+    ps::ps_coef_build_kernel<<<grid_for(c, c->g.cells(), 256), 256, 0, c->stream>>>(
+        c->g, cx, cy, cz, rho_l, rho_g, F_dev, c->ax, c->ay, c->az);
+    c->launches++;
+    PS_CUDA(cudaGetLastError());
+    c->have_coef = true;
+    return PS_OK;
+}
+
+int ps_export_coefficients(ps_ctx *c, double *ax_dev, double *ay_dev, double *az_dev)
+{
+    if (!c) return PS_EINVAL;
+    if (!c->have_coef) return PS_ESTATE;
+    const size_t b = c->g.cells() * sizeof(double);
+    if (ax_dev) PS_CUDA(cudaMemcpyAsync(ax_dev, c->ax, b, cudaMemcpyDeviceToDevice, c->stream));
+    if (ay_dev) PS_CUDA(cudaMemcpyAsync(ay_dev, c->ay, b, cudaMemcpyDeviceToDevice, c->stream));
+    if (az_dev) PS_CUDA(cudaMemcpyAsync(az_dev, c->az, b, cudaMemcpyDeviceToDevice, c->stream));
+    return PS_OK;
+}
+
+int ps_sweeps(ps_ctx *c, const double *rhs_dev, double *p_dev, double omega, int n)
+{
+    if (!c || !rhs_dev || !p_dev || n < 0) return PS_EINVAL;
+    if (!(omega > 0.0 && omega < 2.0)) return PS_EINVAL;
+    if (!c->have_coef) return PS_ESTATE;
+    return run_sweeps(c, rhs_dev, p_dev, omega, n);
+}
+
+int ps_half_sweep(ps_ctx *c, const double *rhs_dev, double *p_dev, double omega, int colour)
+{
+    if (!c || !rhs_dev || !p_dev || (colour != 0 && colour != 1)) return PS_EINVAL;
+    if (!(omega > 0.0 && omega < 2.0)) return PS_EINVAL;
+    if (!c->have_coef) return PS_ESTATE;
+    return launch_half_sweep(c, rhs_dev, p_dev, omega, colour);
+}
+
+int ps_residual(ps_ctx *c, const double *rhs_dev, const double *p_dev, double *res_abs,
+                double *res_rel, double *rhs_norm)
+{
+    if (!c || !rhs_dev || !p_dev || !res_abs) return PS_EINVAL;
+    if (!c->have_coef) return PS_ESTATE;
+    int rc = enqueue_residual(c, rhs_dev, p_dev, 0.0);
+    if (rc) return rc;
+    PS_CUDA(cudaStreamSynchronize(c->stream));
+    *res_abs = c->h_scal[0];
+    if (res_rel) *res_rel = c->h_scal[1];
+    if (rhs_norm) *rhs_norm = c->h_scal[2];
+    return PS_OK;
+}
+
+int ps_solve(ps_ctx *c, const double *rhs_dev, double *p_dev, double omega, int max_sweeps,
+             double tol, ps_info *info)
+{
+    if (!c || !rhs_dev || !p_dev || max_sweeps < 0) return PS_EINVAL;
+    if (!(omega > 0.0 && omega < 2.0)) return PS_EINVAL;
+    if (!c->have_coef) return PS_ESTATE;
+    int s = 0, converged = 0, rc = 0;
+    bool checked = false;
+    if (tol > 0.0) {
+        while (s < max_sweeps) {
+            const int batch = (max_sweeps - s < c->K) ? (max_sweeps - s) : c->K;   // next check
+            rc = run_sweeps(c, rhs_dev, p_dev, omega, batch);
+            if (rc) return rc;
+            s += batch;
+            rc = enqueue_residual(c, rhs_dev, p_dev, tol);
+            if (rc) return rc;
+            PS_CUDA(cudaStreamSynchronize(c->stream));
+            checked = true;
+            if (c->h_scal[1] <= tol) { converged = 1; break; }
+        }
+    } else {
+        rc = run_sweeps(c, rhs_dev, p_dev, omega, max_sweeps);
+        if (rc) return rc;
+        s = max_sweeps;
+    }
+    if (!checked) {
+        rc = enqueue_residual(c, rhs_dev, p_dev, tol);
+        if (rc) return rc;
+        PS_CUDA(cudaStreamSynchronize(c->stream));
+        if (tol > 0.0 && c->h_scal[1] <= tol) converged = 1;
+    }
+    if (info) {
+        info->sweeps = s;
+        info->converged = converged;
+        info->res_abs = c->h_scal[0];
+        info->res_rel = c->h_scal[1];
+        info->rhs_norm = c->h_scal[2];
+    }
+    return PS_OK;
+}
+
+int ps_solve_host(ps_ctx *c, const double *F_host, double rho_l, double rho_g,
+                  const double *rhs_host, double *p_host, double omega, int max_sweeps,
+                  double tol, ps_info *info)
+{
+    if (!c || !F_host || !rhs_host || !p_host) return PS_EINVAL;
+    const size_t b = c->g.cells() * sizeof(double);
+    if (!c->st_F) {
+        cudaError_t e = cudaMalloc((void **)&c->st_F, b);
+        if (e == cudaSuccess) e = cudaMalloc((void **)&c->st_rhs, b);
+        if (e == cudaSuccess) e = cudaMalloc((void **)&c->st_p, b);
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            if (c->st_F) cudaFree(c->st_F);
+            if (c->st_rhs) cudaFree(c->st_rhs);
+            c->st_F = c->st_rhs = c->st_p = nullptr;
+            return e == cudaErrorMemoryAllocation ? PS_ENOMEM : cuda_fail(e);
+        }
+    }
+    PS_CUDA(cudaMemcpyAsync(c->st_F, F_host, b, cudaMemcpyHostToDevice, c->stream));
+    PS_CUDA(cudaMemcpyAsync(c->st_rhs, rhs_host, b, cudaMemcpyHostToDevice, c->stream));
+    PS_CUDA(cudaMemcpyAsync(c->st_p, p_host, b, cudaMemcpyHostToDevice, c->stream));
+    int rc = ps_set_fraction(c, c->st_F, rho_l, rho_g);
+    if (rc) return rc;
+    rc = ps_solve(c, c->st_rhs, c->st_p, omega, max_sweeps, tol, info);
+    if (rc) return rc;
+    PS_CUDA(cudaMemcpyAsync(p_host, c->st_p, b, cudaMemcpyDeviceToHost, c->stream));
+    PS_CUDA(cudaStreamSynchronize(c->stream));
+    return PS_OK;
+}
+
+int ps_enable_timing(ps_ctx *c, int on)
+{
+    if (!c) return PS_EINVAL;
+    c->timing = on != 0;
+    return PS_OK;
+}
+
+int ps_timing(ps_ctx *c, double *sweep_ms, long long *sweep_launches)
+{
+    if (!c) return PS_EINVAL;
+    PS_CUDA(cudaStreamSynchronize(c->stream));
+    double tot = 0.0;
+    for (size_t q = 0; q + 1 < c->ev_used; q += 2) {
+        float ms = 0.f;
+        PS_CUDA(cudaEventElapsedTime(&ms, (*c->ev)[q], (*c->ev)[q + 1]));
+        tot += (double)ms;
+    }
+    if (sweep_ms) *sweep_ms = tot;
+    if (sweep_launches) *sweep_launches = c->timed_launches;
+    c->ev_used = 0;
+    c->timed_launches = 0;
+    return PS_OK;
+}
+
+long long ps_launch_count(const ps_ctx *c) { return c ? c->launches : 0; }
+
+const char *ps_strerror(int code)
+{
+    switch (code) {
+        case PS_OK: return "ok";
+        case PS_EINVAL: return "invalid argument";
+        case PS_ESTATE: return "coefficients not set: call ps_set_fraction first";
+        case PS_ECUDA: return g_cuda_msg;
+        case PS_ENOMEM: return "out of memory";
+        default: return "unknown error code";
+    }
+}
+
+}  // extern "C"

@@ -1,0 +1,236 @@
+// ps_kernels_generic.cuh -- shape-generic CUDA kernels of the pressure-Poisson path (sm_100a).
+//
+//   ps_coef_build_kernel      F -> rho -> ax, ay, az           PAPER.md:66 eq (4), :92, :117, :195
+//   ps_half_sweep_kernel      one colour of red-black SOR
+//   ps_residual_partial_kernel / ps_reduce_final_kernel         DESIGN.md reading S5 (paper silent)
+//
+// These work for any nx, ny >= 1 and even nz >= 2 and are the reference schedule of the CUDA
+// path: one thread per cell (coefficients, residual) or per cell of the active colour (sweep),
+// plain coalesced global loads, neighbour reuse left to L1/L2.  The fast kernels of
+// ps_kernels_fused.cuh compute the same expressions in the same order, so every variant gives
+// bitwise identical p.  Compile with --fmad=false: every * and + below rounds separately.
+#pragma once
+#include <cstddef>
+#include <cstdint>
+
+namespace ps {
+
+struct Grid {
+    int nx, ny, nz;
+    __host__ __device__ size_t cells() const { return (size_t)nx * (size_t)ny * (size_t)nz; }
+    __host__ __device__ size_t idx(int i, int j, int k) const {
+        return (size_t)i + (size_t)nx * ((size_t)j + (size_t)ny * (size_t)k);
+    }
+};
+
+// One SOR update written once, used by every kernel variant.  Argument order = summation order.
+//   s = sum_f a_f p_nb (12 roundings, left to right), d = sum_f a_f, g = (s - rhs)/d,
+//   p <- p + omega (g - p).
+__device__ __forceinline__ double sor_update(double axm, double axp, double aym, double ayp,
+                                             double azm, double azp, double pxm, double pxp,
+                                             double pym, double pyp, double pzm, double pzp,
+                                             double pc, double rhs, double omega)
+{
+    const double s = ((((axm * pxm + axp * pxp) + aym * pym) + ayp * pyp) + azm * pzm) + azp * pzp;
+    const double d = ((((axm + axp) + aym) + ayp) + azm) + azp;
+    const double g = (s - rhs) / d;
+    return pc + omega * (g - pc);
+}
+
+// r_c = rhs_c - (s - d p_c), same s and d.
+__device__ __forceinline__ double residual_at(double axm, double axp, double aym, double ayp,
+                                              double azm, double azp, double pxm, double pxp,
+                                              double pym, double pyp, double pzm, double pzp,
+                                              double pc, double rhs)
+{
+    const double s = ((((axm * pxm + axp * pxp) + aym * pym) + ayp * pyp) + azm * pzm) + azp * pzp;
+    const double d = ((((axm + axp) + aym) + ayp) + azm) + azp;
+    return rhs - (s - d * pc);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Coefficient build: one thread per cell, 8 B in (plus neighbour reads served by L1/L2), 24 B out.
+__global__ void __launch_bounds__(256)
+ps_coef_build_kernel(Grid g, double cx, double cy, double cz, double rho_l, double rho_g,
+                     const double *__restrict__ F, double *__restrict__ ax,
+                     double *__restrict__ ay, double *__restrict__ az)
+{
+    const size_t N = g.cells();
+    const size_t plane = (size_t)g.nx * g.ny;
+    for (size_t n = (size_t)blockIdx.x * blockDim.x + threadIdx.x; n < N;
+         n += (size_t)gridDim.x * blockDim.x) {
+        const int i = (int)(n % g.nx);
+        const size_t t = n / g.nx;
+        const int j = (int)(t % g.ny);
+        const int k = (int)(t / g.ny);
+        const double Fc = F[n];
+        const double rc = (rho_l * Fc) + (rho_g * (1.0 - Fc));
+        double vx = 0.0, vy = 0.0;
+        if (i < g.nx - 1) {
+            const double Fn = F[n + 1];
+            const double rn = (rho_l * Fn) + (rho_g * (1.0 - Fn));
+            vx = cx / (0.5 * (rc + rn));
+        }
+        if (j < g.ny - 1) {
+            const double Fn = F[n + g.nx];
+            const double rn = (rho_l * Fn) + (rho_g * (1.0 - Fn));
+            vy = cy / (0.5 * (rc + rn));
+        }
+        const size_t nz_up = (k + 1 < g.nz) ? n + plane : n - plane * (size_t)(g.nz - 1);
+        const double Fz = F[nz_up];
+        const double rz = (rho_l * Fz) + (rho_g * (1.0 - Fz));
+        ax[n] = vx;
+        ay[n] = vy;
+        az[n] = cz / (0.5 * (rc + rz));
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Gather the six coefficients and neighbour values of cell (i,j,k) from natural-layout arrays.
+// Wall neighbours are read at the clamped index (a finite number) and meet a 0.0 coefficient.
+struct Stencil {
+    double axm, axp, aym, ayp, azm, azp, pxm, pxp, pym, pyp, pzm, pzp;
+};
+
+__device__ __forceinline__ Stencil gather(const Grid &g, const double *__restrict__ ax,
+                                          const double *__restrict__ ay,
+                                          const double *__restrict__ az, const double *p, int i,
+                                          int j, int k, size_t n)
+{
+    const size_t plane = (size_t)g.nx * g.ny;
+    const size_t nzm = (k > 0) ? n - plane : n + plane * (size_t)(g.nz - 1);
+    const size_t nzp = (k + 1 < g.nz) ? n + plane : n - plane * (size_t)(g.nz - 1);
+    Stencil s;
+    s.axm = (i > 0) ? ax[n - 1] : 0.0;
+    s.axp = ax[n];
+    s.aym = (j > 0) ? ay[n - g.nx] : 0.0;
+    s.ayp = ay[n];
+    s.azm = az[nzm];
+    s.azp = az[n];
+    s.pxm = p[(i > 0) ? n - 1 : n];
+    s.pxp = p[(i < g.nx - 1) ? n + 1 : n];
+    s.pym = p[(j > 0) ? n - g.nx : n];
+    s.pyp = p[(j < g.ny - 1) ? n + g.nx : n];
+    s.pzm = p[nzm];
+    s.pzp = p[nzp];
+    return s;
+}
+
+// Half-sweep, in place: one thread per cell of the active colour ((i+j+k)&1 == colour).
+// Cells of one colour never read each other, so no ordering between threads is needed.
+__global__ void __launch_bounds__(256)
+ps_half_sweep_kernel(Grid g, const double *__restrict__ ax, const double *__restrict__ ay,
+                     const double *__restrict__ az, const double *__restrict__ rhs, double *p,
+                     double omega, int colour)
+{
+    const int hx = (g.nx + 1) >> 1;
+    const size_t total = (size_t)hx * g.ny * g.nz;
+    for (size_t h = (size_t)blockIdx.x * blockDim.x + threadIdx.x; h < total;
+         h += (size_t)gridDim.x * blockDim.x) {
+        const int ih = (int)(h % hx);
+        const size_t t = h / hx;
+        const int j = (int)(t % g.ny);
+        const int k = (int)(t / g.ny);
+        const int i = 2 * ih + ((j + k + colour) & 1);
+        if (i >= g.nx) continue;
+        const size_t n = g.idx(i, j, k);
+        const Stencil s = gather(g, ax, ay, az, p, i, j, k, n);
+        p[n] = sor_update(s.axm, s.axp, s.aym, s.ayp, s.azm, s.azp, s.pxm, s.pxp, s.pym, s.pyp,
+                          s.pzm, s.pzp, p[n], rhs[n], omega);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Deterministic two-pass reduction.  Pass 1: block b owns cells [b*CHUNK, (b+1)*CHUNK); thread t
+// adds its cells t, t+256, ... in that order, then a fixed xor-shuffle tree per warp and a fixed
+// left-to-right sum over the 8 warps.  The partition depends on N only (not on the SM count), so
+// the result is reproducible across devices and launches.  No floating-point atomics.
+constexpr int RED_THREADS = 256;
+constexpr int RED_CHUNK = 4096;
+
+__device__ __forceinline__ double warp_tree_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = v + __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+template <int THREADS>
+__device__ __forceinline__ double block_tree_sum(double v, double *smem /* THREADS/32 */)
+{
+    v = warp_tree_sum(v);
+    const int w = threadIdx.x >> 5;
+    if ((threadIdx.x & 31) == 0) smem[w] = v;
+    __syncthreads();
+    double tot = 0.0;
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int q = 0; q < THREADS / 32; ++q) tot = tot + smem[q];
+    }
+    __syncthreads();
+    return tot;   // valid on thread 0
+}
+
+__global__ void __launch_bounds__(RED_THREADS)
+ps_residual_partial_kernel(Grid g, const double *__restrict__ ax, const double *__restrict__ ay,
+                           const double *__restrict__ az, const double *__restrict__ rhs,
+                           const double *__restrict__ p, double *__restrict__ partR2,
+                           double *__restrict__ partB2)
+{
+    __shared__ double sm[RED_THREADS / 32];
+    const size_t N = g.cells();
+    const size_t base = (size_t)blockIdx.x * RED_CHUNK;
+    double r2 = 0.0, b2 = 0.0;
+#pragma unroll 4
+    for (int m = 0; m < RED_CHUNK / RED_THREADS; ++m) {
+        const size_t n = base + (size_t)m * RED_THREADS + threadIdx.x;
+        if (n < N) {
+            const int i = (int)(n % g.nx);
+            const size_t t = n / g.nx;
+            const int j = (int)(t % g.ny);
+            const int k = (int)(t / g.ny);
+            const Stencil s = gather(g, ax, ay, az, p, i, j, k, n);
+            const double b = rhs[n];
+            const double r = residual_at(s.axm, s.axp, s.aym, s.ayp, s.azm, s.azp, s.pxm, s.pxp,
+                                         s.pym, s.pyp, s.pzm, s.pzp, p[n], b);
+            r2 = r2 + r * r;
+            b2 = b2 + b * b;
+        }
+    }
+    const double R = block_tree_sum<RED_THREADS>(r2, sm);
+    const double B = block_tree_sum<RED_THREADS>(b2, sm);
+    if (threadIdx.x == 0) {
+        partR2[blockIdx.x] = R;
+        partB2[blockIdx.x] = B;
+    }
+}
+
+// Pass 2: one block; thread t adds partials t, t+1024, ... in order, then the same fixed tree.
+// out[0] = ||r||_2, out[1] = ||r||_2/||rhs||_2 (||r||_2 if rhs == 0), out[2] = ||rhs||_2.
+// If tol > 0 and out[1] <= tol the device flag done[0] is raised (sweep kernels launched after
+// it may then return at once; see ps_api.cu).
+constexpr int FIN_THREADS = 1024;
+
+__global__ void __launch_bounds__(FIN_THREADS)
+ps_reduce_final_kernel(const double *__restrict__ partR2, const double *__restrict__ partB2,
+                       int nparts, double tol, double *__restrict__ out, int *done)
+{
+    __shared__ double sm[FIN_THREADS / 32];
+    double r2 = 0.0, b2 = 0.0;
+    for (int q = threadIdx.x; q < nparts; q += FIN_THREADS) {
+        r2 = r2 + partR2[q];
+        b2 = b2 + partB2[q];
+    }
+    const double R = block_tree_sum<FIN_THREADS>(r2, sm);
+    const double B = block_tree_sum<FIN_THREADS>(b2, sm);
+    if (threadIdx.x == 0) {
+        const double ra = sqrt(R), bn = sqrt(B);
+        const double rr = (bn > 0.0) ? ra / bn : ra;
+        out[0] = ra;
+        out[1] = rr;
+        out[2] = bn;
+        if (done != nullptr && tol > 0.0 && rr <= tol) done[0] = 1;
+    }
+}
+
+}  // namespace ps

@@ -1,0 +1,334 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element, on the
+same seeded inputs.  Bar (BASELINE.json north_star): max-rel p <= 1e-12 after N sweeps, residual
+norms <= 1e-10 relative.  Because both sides round the same expressions in the same order
+(--fmad=false / -ffp-contract=off) and red-black SOR is schedule independent, the expectation is
+ZERO differing doubles; both are asserted.
+"""
+import numpy as np
+import pytest
+
+from paper_2104_01636_b200 import workload as wl
+
+pytestmark = pytest.mark.gpu
+
+P_TOL = 1e-12       # max_n |p_gpu - p_ora| / max_n |p_ora|
+NORM_TOL = 1e-10    # |res_gpu - res_ora| / res_ora
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "these tests need the B200"
+    return torch
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2104_01636_b200 import binding, build
+    build.build()
+    binding.load()          # fails loudly if the CUDA extension is missing
+    return binding
+
+
+def to_dev(torch, a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def assert_p_parity(p_gpu, p_ora, what=""):
+    scale = np.max(np.abs(p_ora))
+    diff = np.max(np.abs(p_gpu - p_ora)) / (scale if scale > 0 else 1.0)
+    nbad = int(np.count_nonzero(p_gpu != p_ora))
+    assert diff <= P_TOL, f"{what}: max-rel p diff {diff:.3e}"
+    assert nbad == 0, f"{what}: {nbad} doubles differ (max-rel {diff:.3e})"
+
+
+def variants_for(B, w):
+    """Kernel variants the library accepts for this grid shape (asked of the library itself)."""
+    out = []
+    with B.PoissonSolver(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, workspace=False) as s:
+        for v in (B.KERNEL_TWOPASS, B.KERNEL_FUSED, B.KERNEL_FUSED_T2):
+            try:
+                s.set_kernel(v)
+                out.append(v)
+            except B.PsError:
+                pass
+    return out
+
+
+def make_solver(B, w, variant=None):
+    s = B.PoissonSolver(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz)
+    if variant is not None:
+        s.set_kernel(variant)
+    return s
+
+
+SHAPES = [
+    # nx, ny, nz, spheres, diameter, (dx, dy, dz)
+    (16, 12, 20, 0, 0, (0.1, 0.07, 0.13)),       # anisotropic spacing, tiny
+    (1, 1, 8, 0, 0, None),                       # 1-D periodic degenerate case
+    (5, 7, 6, 0, 0, None),                       # odd nx, ny
+    (2, 3, 2, 0, 0, None),                       # smallest legal nz
+    (40, 36, 24, 2, 8, None),                    # spheres, several tiles + ragged tails
+    (72, 52, 34, 3, 12, (1 / 72, 1 / 60, 1 / 50)),
+    (132, 20, 10, 0, 0, None),                   # wider than one x tile
+]
+
+
+def shape_workload(nx, ny, nz, count, diam, h, seed=11):
+    kw = {}
+    if h is not None:
+        kw = dict(dx=h[0], dy=h[1], dz=h[2])
+    w = wl.make_custom(nx, ny, nz, count, diam, seed, **kw)
+    if count == 0:                                # hardest coefficients: random F in {m/64}
+        w.F = wl.random_fraction(nx, ny, nz, seed)
+    return w
+
+
+# ---------------------------------------------------------------- (a1) coefficient build
+@pytest.mark.parametrize("shape", SHAPES)
+def test_coefficients_bitwise(torch_cuda, B, ora, shape):
+    w = shape_workload(*shape)
+    ax, ay, az = ora.coefficients(w.F, w.rho_l, w.rho_g, w.dx, w.dy, w.dz)
+    with make_solver(B, w) as s:
+        s.set_fraction(to_dev(torch_cuda, w.F), w.rho_l, w.rho_g)
+        gx, gy, gz = [t.cpu().numpy() for t in s.export_coefficients()]
+    assert np.array_equal(gx, ax) and np.array_equal(gy, ay) and np.array_equal(gz, az)
+
+
+# ---------------------------------------------------------------- (a2)/(a3) half-sweeps
+@pytest.mark.parametrize("shape", SHAPES[:5])
+def test_half_sweeps_bitwise(torch_cuda, B, ora, shape):
+    w = shape_workload(*shape)
+    coef = ora.coefficients(w.F, w.rho_l, w.rho_g, w.dx, w.dy, w.dz)
+    p0 = wl.noise_rhs(w.nx, w.ny, w.nz, 99)       # non-trivial start
+    with make_solver(B, w) as s:
+        s.set_fraction(to_dev(torch_cuda, w.F), w.rho_l, w.rho_g)
+        rhs_d = to_dev(torch_cuda, w.rhs)
+        for colour in (0, 1):
+            p_ora = p0.copy()
+            ora.half_sweep(coef, w.rhs, p_ora, w.omega, colour)
+            p_d = to_dev(torch_cuda, p0)
+            s.half_sweep(rhs_d, p_d, w.omega, colour)
+            assert_p_parity(p_d.cpu().numpy(), p_ora, f"colour {colour}")
+            other = ((np.add.outer(np.add.outer(np.arange(w.nz), np.arange(w.ny)),
+                                   np.arange(w.nx)) & 1) != colour)
+            assert np.array_equal(p_d.cpu().numpy()[other], p0[other])   # other colour untouched
+
+
+# ---------------------------------------------------------------- sweeps, every kernel variant
+@pytest.mark.parametrize("nsweeps", [1, 2, 3, 7])
+@pytest.mark.parametrize("shape", SHAPES)
+def test_sweeps_bitwise_all_variants(torch_cuda, B, ora, shape, nsweeps):
+    w = shape_workload(*shape)
+    coef = ora.coefficients(w.F, w.rho_l, w.rho_g, w.dx, w.dy, w.dz)
+    p_ora = np.zeros_like(w.rhs)
+    ora.sweep(coef, w.rhs, p_ora, w.omega, nsweeps)
+    ra, rr, bn = ora.residual(coef, w.rhs, p_ora)
+    for variant in variants_for(B, w):
+        with make_solver(B, w, variant) as s:
+            s.set_fraction(to_dev(torch_cuda, w.F), w.rho_l, w.rho_g)
+            rhs_d = to_dev(torch_cuda, w.rhs)
+            p_d = torch_cuda.zeros_like(rhs_d)
+            s.sweeps(rhs_d, p_d, w.omega, nsweeps)
+            assert_p_parity(p_d.cpu().numpy(), p_ora, f"variant {variant} x{nsweeps}")
+            ga, gr, gb = s.residual(rhs_d, p_d)
+        assert abs(ga - ra) <= NORM_TOL * ra and abs(gr - rr) <= NORM_TOL * rr
+        assert abs(gb - bn) <= NORM_TOL * bn
+
+
+# ---------------------------------------------------------------- BASELINE.json configs
+def test_config1_200_sweeps(torch_cuda, B, ora):
+    """configs[0]: 32x32x64, one D=8 sphere, omega 1.5, 200 sweeps -- p and norms."""
+    w = wl.make_config(1)
+    coef = ora.coefficients(w.F, w.rho_l, w.rho_g, w.dx, w.dy, w.dz)
+    p_ora = np.zeros_like(w.rhs)
+    io = ora.solve(coef, w.rhs, p_ora, w.omega, w.max_sweeps, 0.0)
+    for variant in variants_for(B, w):
+        with make_solver(B, w, variant) as s:
+            s.set_fraction(to_dev(torch_cuda, w.F), w.rho_l, w.rho_g)
+            rhs_d = to_dev(torch_cuda, w.rhs)
+            p_d = torch_cuda.zeros_like(rhs_d)
+            ig = s.solve(rhs_d, p_d, w.omega, w.max_sweeps, 0.0)
+            assert_p_parity(p_d.cpu().numpy(), p_ora, f"config1 variant {variant}")
+        assert ig.sweeps == io.sweeps == 200 and not ig.converged
+        assert abs(ig.res_abs - io.res_abs) <= NORM_TOL * io.res_abs
+        assert abs(ig.res_rel - io.res_rel) <= NORM_TOL * io.res_rel
+        assert abs(ig.rhs_norm - io.rhs_norm) <= NORM_TOL * io.rhs_norm
+
+
+def test_config2_to_tolerance(torch_cuda, B, ora):
+    """configs[1]: unladen 64x64x128, omega 1.7, to 1e-8: same sweep count, p, norms; and the
+    converged field is the eigenmode / lambda (closed form) up to the 1e-3 noise."""
+    w = wl.make_config(2)
+    coef = ora.coefficients(w.F, w.rho_l, w.rho_g, w.dx, w.dy, w.dz)
+    p_ora = np.zeros_like(w.rhs)
+    io = ora.solve(coef, w.rhs, p_ora, w.omega, 100000, w.tol)
+    assert io.converged
+    for variant in variants_for(B, w):
+        with make_solver(B, w, variant) as s:
+            s.set_fraction(to_dev(torch_cuda, w.F), w.rho_l, w.rho_g)
+            rhs_d = to_dev(torch_cuda, w.rhs)
+            p_d = torch_cuda.zeros_like(rhs_d)
+            ig = s.solve(rhs_d, p_d, w.omega, 100000, w.tol)
+            p_gpu = p_d.cpu().numpy()
+        assert ig.converged and ig.sweeps == io.sweeps
+        assert_p_parity(p_gpu, p_ora, f"config2 variant {variant}")
+        assert abs(ig.res_rel - io.res_rel) <= NORM_TOL * io.res_rel
+        assert ig.res_rel <= w.tol
+    import json, os
+    with open(os.path.join(os.path.dirname(__file__), "golden", "eigenvalue_config2.json")) as f:
+        lam = json.load(f)["lambda_1_2_3"]
+    mode = wl.eigenmode(w.nx, w.ny, w.nz, 1, 2, 3) / lam
+    q = p_gpu - p_gpu.mean()
+    assert np.max(np.abs(q - mode)) <= 2e-2 * np.max(np.abs(mode))
+
+
+def test_config3_fixed_sweeps(torch_cuda, B, ora):
+    """configs[2]: 128x128x256, 108 spheres D=12, omega 1.6 -- bitwise parity at 60 sweeps."""
+    w = wl.make_config(3)
+    coef = ora.coefficients(w.F, w.rho_l, w.rho_g, w.dx, w.dy, w.dz)
+    p_ora = np.zeros_like(w.rhs)
+    n = 60
+    io = ora.solve(coef, w.rhs, p_ora, w.omega, n, 0.0)
+    for variant in variants_for(B, w):
+        with make_solver(B, w, variant) as s:
+            s.set_fraction(to_dev(torch_cuda, w.F), w.rho_l, w.rho_g)
+            gx, gy, gz = [t.cpu().numpy() for t in s.export_coefficients()]
+            assert np.array_equal(gx, coef[0]) and np.array_equal(gy, coef[1])
+            assert np.array_equal(gz, coef[2])
+            rhs_d = to_dev(torch_cuda, w.rhs)
+            p_d = torch_cuda.zeros_like(rhs_d)
+            ig = s.solve(rhs_d, p_d, w.omega, n, 0.0)
+            assert_p_parity(p_d.cpu().numpy(), p_ora, f"config3 variant {variant}")
+        assert abs(ig.res_rel - io.res_rel) <= NORM_TOL * io.res_rel
+
+
+@pytest.mark.parametrize("cfg,nsweeps", [(4, 500), (5, 24)])
+def test_full_size_configs(torch_cuda, B, ora, cfg, nsweeps):
+    """configs[3] (256x256x512, 864 spheres, its full 500 sweeps) and configs[4] (384x384x1024,
+    2048 spheres; 24 of its 300 sweeps -- what the oracle does in ~10 s) at full size in the launch
+    configuration bench.py times (kernel AUTO): full-field bitwise parity of p and the norms, then
+    two properties that hold at any size: the norm ps_solve reports equals a fresh ps_residual,
+    and rolling the inputs by an even number of z planes rolls p bitwise (pin P7)."""
+    w = wl.make_config(cfg)
+    coef = ora.coefficients(w.F, w.rho_l, w.rho_g, w.dx, w.dy, w.dz)
+    p_ora = np.zeros_like(w.rhs)
+    io = ora.solve(coef, w.rhs, p_ora, w.omega, nsweeps, 0.0)
+    del coef
+    with make_solver(B, w) as s:
+        F_d, rhs_d = to_dev(torch_cuda, w.F), to_dev(torch_cuda, w.rhs)
+        s.set_fraction(F_d, w.rho_l, w.rho_g)
+        p_d = torch_cuda.zeros_like(rhs_d)
+        ig = s.solve(rhs_d, p_d, w.omega, nsweeps, 0.0)
+        assert_p_parity(p_d.cpu().numpy(), p_ora, f"config{cfg}")
+        del p_ora
+        assert abs(ig.res_rel - io.res_rel) <= NORM_TOL * io.res_rel
+        assert abs(ig.rhs_norm - io.rhs_norm) <= NORM_TOL * io.rhs_norm
+        ra, rr, bn = s.residual(rhs_d, p_d)
+        assert ig.sweeps == nsweeps and (ra, rr, bn) == (ig.res_abs, ig.res_rel, ig.rhs_norm)
+        shift = 6
+        s.set_fraction(torch_cuda.roll(F_d, shift, 0).contiguous(), w.rho_l, w.rho_g)
+        q_d = torch_cuda.zeros_like(rhs_d)
+        s.solve(torch_cuda.roll(rhs_d, shift, 0).contiguous(), q_d, w.omega, nsweeps, 0.0)
+        assert torch_cuda.equal(torch_cuda.roll(p_d, shift, 0), q_d)
+
+
+# ---------------------------------------------------------------- solve loop and API behaviour
+def test_solve_check_cadence_matches_oracle(torch_cuda, B, ora):
+    """Stops at the first check (every K sweeps and at max_sweeps) with res_rel <= tol."""
+    w = shape_workload(16, 12, 20, 0, 0, None)
+    w.F[:] = 1.0
+    coef = ora.coefficients(w.F, w.rho_l, w.rho_g, w.dx, w.dy, w.dz)
+    for K, max_sweeps, tol in [(7, 1000, 1e-6), (50, 33, 1e-30), (10, 1000, 1e-9), (3, 0, 1e-3)]:
+        p_ora = np.zeros_like(w.rhs)
+        io = ora.solve(coef, w.rhs, p_ora, 1.5, max_sweeps, tol, check_interval=K)
+        with make_solver(B, w) as s:
+            s.set_check_interval(K)
+            s.set_fraction(to_dev(torch_cuda, w.F), w.rho_l, w.rho_g)
+            rhs_d = to_dev(torch_cuda, w.rhs)
+            p_d = torch_cuda.zeros_like(rhs_d)
+            ig = s.solve(rhs_d, p_d, 1.5, max_sweeps, tol)
+            assert (ig.sweeps, ig.converged) == (io.sweeps, io.converged), (K, max_sweeps, tol)
+            assert_p_parity(p_d.cpu().numpy(), p_ora)
+            assert abs(ig.res_rel - io.res_rel) <= NORM_TOL * io.res_rel
+
+
+def test_warm_start_and_restart(torch_cuda, B, ora):
+    """p is in/out: 5 sweeps + 6 sweeps == 11 sweeps, bitwise, for every variant."""
+    w = shape_workload(40, 36, 24, 2, 8, None)
+    for variant in variants_for(B, w):
+        with make_solver(B, w, variant) as s:
+            s.set_fraction(to_dev(torch_cuda, w.F), w.rho_l, w.rho_g)
+            rhs_d = to_dev(torch_cuda, w.rhs)
+            a = torch_cuda.zeros_like(rhs_d)
+            s.sweeps(rhs_d, a, w.omega, 5)
+            s.sweeps(rhs_d, a, w.omega, 6)
+            b = torch_cuda.zeros_like(rhs_d)
+            s.sweeps(rhs_d, b, w.omega, 11)
+            assert torch_cuda.equal(a, b)
+
+
+def test_deterministic_norm(torch_cuda, B):
+    """The two-pass reduction has a fixed summation tree: repeated calls agree to the last bit."""
+    w = shape_workload(72, 52, 34, 3, 12, None)
+    with make_solver(B, w) as s:
+        s.set_fraction(to_dev(torch_cuda, w.F), w.rho_l, w.rho_g)
+        rhs_d = to_dev(torch_cuda, w.rhs)
+        p_d = torch_cuda.zeros_like(rhs_d)
+        s.sweeps(rhs_d, p_d, w.omega, 3)
+        vals = {s.residual(rhs_d, p_d) for _ in range(5)}
+    assert len(vals) == 1
+
+
+def test_zero_rhs_and_state_errors(torch_cuda, B):
+    w = shape_workload(16, 12, 20, 0, 0, None)
+    with make_solver(B, w) as s:
+        rhs_d = torch_cuda.zeros(w.nz, w.ny, w.nx, dtype=torch_cuda.float64, device="cuda")
+        p_d = torch_cuda.zeros_like(rhs_d)
+        with pytest.raises(B.PsError) as e:
+            s.solve(rhs_d, p_d, 1.5, 1, 0.0)          # before set_fraction
+        assert e.value.code == B.PS_ESTATE
+        s.set_fraction(to_dev(torch_cuda, w.F), w.rho_l, w.rho_g)
+        info = s.solve(rhs_d, p_d, 1.5, 3, 1e-8)      # rhs = 0, p = 0: residual 0, rel := abs
+        assert info.res_abs == 0.0 and info.res_rel == 0.0 and info.rhs_norm == 0.0
+        assert info.converged and float(p_d.abs().max()) == 0.0
+        for bad_omega in (0.0, 2.0, -1.0, float("nan")):
+            with pytest.raises(B.PsError) as e:
+                s.solve(rhs_d, p_d, bad_omega, 1, 0.0)
+            assert e.value.code == B.PS_EINVAL
+        with pytest.raises(B.PsError):
+            s.solve(rhs_d, p_d, 1.5, -1, 0.0)
+        with pytest.raises(B.PsError):
+            s.set_fraction(to_dev(torch_cuda, w.F), -1.0, 1.2)
+        assert s.launch_count() > 0
+
+
+def test_solve_host_end_to_end(torch_cuda, B, ora):
+    """ps_solve_host: host buffers in, host p out -- same numbers as the device-pointer path."""
+    w = wl.make_config(1)
+    coef = ora.coefficients(w.F, w.rho_l, w.rho_g, w.dx, w.dy, w.dz)
+    p_ora = np.zeros_like(w.rhs)
+    io = ora.solve(coef, w.rhs, p_ora, w.omega, 40, 0.0)
+    p = np.zeros_like(w.rhs)
+    with make_solver(B, w) as s:
+        ig = s.solve_host(w.F, w.rho_l, w.rho_g, w.rhs, p, w.omega, 40, 0.0)
+    assert_p_parity(p, p_ora, "solve_host")
+    assert abs(ig.res_rel - io.res_rel) <= NORM_TOL * io.res_rel
+
+
+def test_non_default_stream_and_library_workspace(torch_cuda, B, ora):
+    w = shape_workload(40, 36, 24, 2, 8, None)
+    coef = ora.coefficients(w.F, w.rho_l, w.rho_g, w.dx, w.dy, w.dz)
+    p_ora = np.zeros_like(w.rhs)
+    ora.sweep(coef, w.rhs, p_ora, w.omega, 4)
+    s = B.PoissonSolver(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, workspace=False)   # cudaMalloc'd ws
+    st = torch_cuda.cuda.Stream()
+    F_d, rhs_d = to_dev(torch_cuda, w.F), to_dev(torch_cuda, w.rhs)
+    p_d = torch_cuda.zeros_like(rhs_d)
+    torch_cuda.cuda.synchronize()
+    with torch_cuda.cuda.stream(st):
+        s.set_fraction(F_d, w.rho_l, w.rho_g)
+        s.sweeps(rhs_d, p_d, w.omega, 4)
+    st.synchronize()
+    assert_p_parity(p_d.cpu().numpy(), p_ora, "side stream")
+    s.close()
