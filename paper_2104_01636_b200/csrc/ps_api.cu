@@ -101,9 +101,10 @@ int ensure_workspace(ps_ctx *c)
 
 int resolve_variant(const ps_ctx *c, int req)
 {
-    const bool fused_ok = ps::fused_shape_ok(c->g);
+    const bool fused_ok = c->fused.ok;
     if (req == PS_KERNEL_AUTO) return fused_ok ? PS_KERNEL_FUSED : PS_KERNEL_TWOPASS;
-    if ((req == PS_KERNEL_FUSED || req == PS_KERNEL_FUSED_T2) && !fused_ok) return -1;
+    if (req == PS_KERNEL_FUSED && !fused_ok) return -1;
+    if (req == PS_KERNEL_FUSED_T2) return -1;          // not built yet
     if (req < PS_KERNEL_AUTO || req > PS_KERNEL_FUSED_T2) return -1;
     return req;
 }
@@ -223,12 +224,18 @@ int ps_create(ps_ctx **out, int nx, int ny, int nz, double dx, double dy, double
     c->K = 50;
     c->sm_count = sms;
     c->nparts = (int)((c->g.cells() + ps::RED_CHUNK - 1) / ps::RED_CHUNK);
+    cudaError_t e = cudaMallocHost((void **)&c->h_scal, 4 * sizeof(double));
+    if (e != cudaSuccess) { delete c->ev; delete c; return cuda_fail(e); }
+    e = ps::fused_plan_init(&c->fused, c->g, sms);
+    if (e != cudaSuccess) {
+        ps::fused_plan_destroy(&c->fused);
+        cudaFreeHost(c->h_scal);
+        delete c->ev;
+        delete c;
+        return cuda_fail(e);
+    }
     c->variant_req = PS_KERNEL_AUTO;
     c->variant = resolve_variant(c, PS_KERNEL_AUTO);
-    cudaError_t e = cudaMallocHost((void **)&c->h_scal, 4 * sizeof(double));
-    if (e != cudaSuccess) { delete c; return cuda_fail(e); }
-    e = ps::fused_plan_init(&c->fused, c->g, sms);
-    if (e != cudaSuccess) { cudaFreeHost(c->h_scal); delete c; return cuda_fail(e); }
     *out = c;
     return PS_OK;
 }
@@ -238,6 +245,7 @@ int ps_destroy(ps_ctx *c)
     if (!c) return PS_OK;
     if (c->ws && c->ws_owned) cudaFree(c->ws);
     if (c->h_scal) cudaFreeHost(c->h_scal);
+    ps::fused_plan_destroy(&c->fused);
     if (c->st_F) cudaFree(c->st_F);
     if (c->st_rhs) cudaFree(c->st_rhs);
     if (c->st_p) cudaFree(c->st_p);
