@@ -54,6 +54,8 @@ def parse_args():
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json config 1..5 (default 4)")
     ap.add_argument("--sweeps", type=int, default=0, help="sweeps per step (default: the config's)")
     ap.add_argument("--kernel", default="auto", choices=["auto", "twopass", "fused", "fused_t2"])
+    ap.add_argument("--rpt", type=int, default=0, help="fused kernel: rows per thread (0 = auto)")
+    ap.add_argument("--zchunks", type=int, default=0, help="fused kernel: z chunks (0 = auto)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="oracle sample budget")
@@ -231,6 +233,11 @@ def run_ours(args, rank):
     s = binding.PoissonSolver(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz)
     s.set_kernel(kernel)
     kname = binding.KERNEL_NAMES[s.get_kernel()]
+    tuning = None
+    if kname != "twopass":
+        if args.rpt or args.zchunks:
+            s.set_tuning(args.rpt, args.zchunks)
+        tuning = dict(zip(("rows_per_thread", "z_chunks", "tiles"), s.get_tuning()))
 
     def step():
         p_d.zero_()
@@ -297,7 +304,7 @@ def run_ours(args, rank):
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic",
         "config": {"workload": w.name, "cells": w.cells, "sweeps_per_step": sweeps,
-                   "omega": w.omega, "kernel": kname, "spheres": int(len(w.centres)),
+                   "omega": w.omega, "kernel": kname, "tuning": tuning, "spheres": int(len(w.centres)),
                    "step": "ps_set_fraction + ps_solve(sweeps, tol=0) incl. residual",
                    "l2": "working set 1.3 GB+ >> 126 MB L2 (no flush needed)" if w.cells > 8e6
                          else "L2-resident working set (not an HBM measurement)",

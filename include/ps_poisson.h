@@ -87,9 +87,17 @@ int ps_set_stream(ps_ctx *c, void *cuda_stream);
 int ps_set_check_interval(ps_ctx *c, int K);
 
 /* Choose the sweep kernel (PS_KERNEL_*).  PS_EINVAL if the grid shape does not allow the
- * variant (the fused kernels need nx % 4 == 0, nx >= 8, ny >= 4, nz >= 4). */
+ * variant (the fused kernels need nx even). */
 int ps_set_kernel(ps_ctx *c, int variant);
 int ps_get_kernel(const ps_ctx *c);          /* the variant AUTO resolved to, or the one set */
+
+/* Launch geometry of the fused kernel (tuning and tests; every setting gives bitwise identical p).
+ * rows_per_thread: 1 = 64x16-cell boxes, 2 = 64x32-cell boxes, 0 = keep.  z_chunks: number of
+ * z chunks each (x,y) tile is cut into (CTAs = tiles * z_chunks), 0 = choose by the cost model
+ * (rounds of sm_count CTAs x (planes per chunk + z halo)).  Synchronises the stream.
+ * PS_EINVAL: fused kernel not available for this grid, values out of range. */
+int ps_set_tuning(ps_ctx *c, int rows_per_thread, int z_chunks);
+int ps_get_tuning(const ps_ctx *c, int *rows_per_thread, int *z_chunks, int *tiles);
 
 /* Step 4 of the paper's time step + face coefficients:
  * rho = rho_l F + rho_g (1-F); ax,ay,az = (1/h^2)/(0.5 (rho_c + rho_nb)) for the +x,+y,+z

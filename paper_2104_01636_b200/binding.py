@@ -22,7 +22,8 @@ KERNEL_NAMES = {KERNEL_AUTO: "auto", KERNEL_TWOPASS: "twopass", KERNEL_FUSED: "f
 
 # every symbol include/ps_poisson.h declares (tests check the library exports each one)
 SYMBOLS = ("ps_create", "ps_destroy", "ps_workspace_bytes", "ps_set_workspace", "ps_set_stream",
-           "ps_set_check_interval", "ps_set_kernel", "ps_get_kernel", "ps_set_fraction",
+           "ps_set_check_interval", "ps_set_kernel", "ps_get_kernel", "ps_set_tuning",
+           "ps_get_tuning", "ps_set_fraction",
            "ps_export_coefficients", "ps_solve", "ps_sweeps", "ps_half_sweep", "ps_residual",
            "ps_solve_host", "ps_enable_timing", "ps_timing", "ps_launch_count", "ps_strerror")
 
@@ -71,6 +72,9 @@ def load(path: str | None = None) -> ctypes.CDLL:
     lib.ps_set_check_interval.argtypes = [vp, i]
     lib.ps_set_kernel.argtypes = [vp, i]
     lib.ps_get_kernel.argtypes = [vp]
+    lib.ps_set_tuning.argtypes = [vp, i, i]
+    ip = ctypes.POINTER(ctypes.c_int)
+    lib.ps_get_tuning.argtypes = [vp, ip, ip, ip]
     lib.ps_set_fraction.argtypes = [vp, vp, d, d]
     lib.ps_export_coefficients.argtypes = [vp, vp, vp, vp]
     lib.ps_solve.argtypes = [vp, vp, vp, d, i, d, ctypes.POINTER(_Info)]
@@ -166,6 +170,16 @@ class PoissonSolver:
 
     def get_kernel(self) -> int:
         return self._lib.ps_get_kernel(self._h)
+
+    def set_tuning(self, rows_per_thread: int = 0, z_chunks: int = 0):
+        _check(self._lib, self._lib.ps_set_tuning(self._h, rows_per_thread, z_chunks))
+
+    def get_tuning(self):
+        """(rows_per_thread, z_chunks, tiles) of the fused kernel's launch geometry."""
+        a, b, c = ctypes.c_int(), ctypes.c_int(), ctypes.c_int()
+        _check(self._lib, self._lib.ps_get_tuning(self._h, ctypes.byref(a), ctypes.byref(b),
+                                                  ctypes.byref(c)))
+        return a.value, b.value, c.value
 
     def workspace_bytes(self) -> int:
         return self._lib.ps_workspace_bytes(self._h)

@@ -12,7 +12,7 @@
 
 #include "../../include/ps_poisson.h"
 #include "ps_kernels_generic.cuh"
-#include "ps_kernels_fused.cuh"
+#include "ps_kernels_zmarch.cuh"
 
 namespace {
 
@@ -54,7 +54,7 @@ struct ps_ctx {
     double *h_scal;        // pinned, 4 doubles
     // staging of ps_solve_host
     double *st_F, *st_rhs, *st_p;
-    ps::FusedPlan fused;
+    ps::ZmPlan fused;
     // optional event timing of the sweep launches (ps_enable_timing)
     bool timing;
     std::vector<cudaEvent_t> *ev;      // pairs: start, stop
@@ -167,13 +167,11 @@ int run_sweeps_untimed(ps_ctx *c, const double *rhs, double *p, double omega, in
     double *src = p, *dst = c->p_alt;
     int left = n;
     while (left > 0) {
-        int did = 0;
-        cudaError_t e = ps::launch_fused(c->fused, c->g, c->ax, c->ay, c->az, rhs, src, dst, omega,
-                                         (c->variant == PS_KERNEL_FUSED_T2 && left >= 2) ? 2 : 1,
-                                         c->stream, &did);
+        cudaError_t e = ps::zm_launch(c->fused, c->g, c->ax, c->ay, c->az, rhs, src, dst, omega,
+                                      c->stream);
         c->launches++;
         if (e != cudaSuccess) return cuda_fail(e);
-        left -= did;
+        left -= 1;
         double *t = src; src = dst; dst = t;
     }
     if (src != p) {
@@ -226,9 +224,9 @@ int ps_create(ps_ctx **out, int nx, int ny, int nz, double dx, double dy, double
     c->nparts = (int)((c->g.cells() + ps::RED_CHUNK - 1) / ps::RED_CHUNK);
     cudaError_t e = cudaMallocHost((void **)&c->h_scal, 4 * sizeof(double));
     if (e != cudaSuccess) { delete c->ev; delete c; return cuda_fail(e); }
-    e = ps::fused_plan_init(&c->fused, c->g, sms);
+    e = ps::zm_plan_init(&c->fused, c->g, sms);
     if (e != cudaSuccess) {
-        ps::fused_plan_destroy(&c->fused);
+        ps::zm_plan_destroy(&c->fused);
         cudaFreeHost(c->h_scal);
         delete c->ev;
         delete c;
@@ -245,7 +243,7 @@ int ps_destroy(ps_ctx *c)
     if (!c) return PS_OK;
     if (c->ws && c->ws_owned) cudaFree(c->ws);
     if (c->h_scal) cudaFreeHost(c->h_scal);
-    ps::fused_plan_destroy(&c->fused);
+    ps::zm_plan_destroy(&c->fused);
     if (c->st_F) cudaFree(c->st_F);
     if (c->st_rhs) cudaFree(c->st_rhs);
     if (c->st_p) cudaFree(c->st_p);
@@ -297,6 +295,28 @@ int ps_set_kernel(ps_ctx *c, int variant)
 }
 
 int ps_get_kernel(const ps_ctx *c) { return c ? c->variant : PS_EINVAL; }
+
+int ps_set_tuning(ps_ctx *c, int rows_per_thread, int z_chunks)
+{
+    if (!c || !c->fused.ok) return PS_EINVAL;
+    if (rows_per_thread < 0 || rows_per_thread > 2 || z_chunks < 0 || z_chunks > c->g.nz / 2)
+        return PS_EINVAL;
+    const int rpt = rows_per_thread ? rows_per_thread : c->fused.rpt;
+    PS_CUDA(cudaStreamSynchronize(c->stream));
+    const cudaError_t e = ps::zm_plan_tiles(&c->fused, c->g, rpt, z_chunks);
+    if (e == cudaErrorInvalidValue) { cudaGetLastError(); return PS_EINVAL; }
+    if (e != cudaSuccess) return cuda_fail(e);
+    return PS_OK;
+}
+
+int ps_get_tuning(const ps_ctx *c, int *rows_per_thread, int *z_chunks, int *tiles)
+{
+    if (!c || !c->fused.ok) return PS_EINVAL;
+    if (rows_per_thread) *rows_per_thread = c->fused.rpt;
+    if (z_chunks) *z_chunks = c->fused.nchunks;
+    if (tiles) *tiles = c->fused.ntiles;
+    return PS_OK;
+}
 
 int ps_set_fraction(ps_ctx *c, const double *F_dev, double rho_l, double rho_g)
 {

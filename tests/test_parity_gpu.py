@@ -42,23 +42,35 @@ def assert_p_parity(p_gpu, p_ora, what=""):
     assert nbad == 0, f"{what}: {nbad} doubles differ (max-rel {diff:.3e})"
 
 
-def variants_for(B, w):
-    """Kernel variants the library accepts for this grid shape (asked of the library itself)."""
+def variants_for(B, w, tunings=((1, 0), (2, 0), (1, 1), (2, 3))):
+    """Kernel variants the library accepts for this grid shape (asked of the library itself):
+    (kernel, rows_per_thread, z_chunks); the fused kernel is run in several launch geometries."""
     out = []
     with B.PoissonSolver(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, workspace=False) as s:
         for v in (B.KERNEL_TWOPASS, B.KERNEL_FUSED, B.KERNEL_FUSED_T2):
             try:
                 s.set_kernel(v)
-                out.append(v)
             except B.PsError:
-                pass
+                continue
+            if v == B.KERNEL_TWOPASS:
+                out.append((v, 0, 0))
+                continue
+            for rpt, chunks in tunings:
+                try:
+                    s.set_tuning(rpt, chunks)
+                    out.append((v, rpt, chunks))
+                except B.PsError:
+                    pass
     return out
 
 
 def make_solver(B, w, variant=None):
     s = B.PoissonSolver(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz)
     if variant is not None:
-        s.set_kernel(variant)
+        kernel, rpt, chunks = variant
+        s.set_kernel(kernel)
+        if kernel != B.KERNEL_TWOPASS:
+            s.set_tuning(rpt, chunks)
     return s
 
 
