@@ -1,0 +1,102 @@
+"""Five-config report of the CUDA path (BASELINE.json `metric`):
+
+    python -m paper_2104_01636_b200.report [--configs 1,2,3,4,5] [--max-sweeps 1000000] [--md FILE]
+
+For every config: fixed-sweep throughput (Gcell-updates/s, CUDA events around `ps_sweeps`), the
+model HBM rate of the kernel that ran (bytes per cell-update of DESIGN.md §7 x throughput), and --
+for every config but the largest -- wall time and sweep count of `ps_solve` to a relative
+residual of 1e-8 (check cadence K = 50, norm checks and the final read-back included).  Prints a
+markdown table.  Needs the B200 and the built library: there is no CPU path.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import sys
+import time
+
+BYTES_PER_UPDATE = {"twopass": 80.0, "fused": 48.0, "fused_t2": 24.0}
+
+
+def run_config(cfg: int, max_sweeps: int, to_tol: bool, kernel: int):
+    import torch
+    from . import binding, workload as wl
+    w = wl.make_config(cfg)
+    fixed = wl.CONFIGS[cfg][7] or 500
+    F_d = torch.from_numpy(w.F).cuda()
+    rhs_d = torch.from_numpy(w.rhs).cuda()
+    p_d = torch.zeros_like(rhs_d)
+    out = {"config": cfg, "workload": w.name, "cells": w.cells, "omega": w.omega}
+    with binding.PoissonSolver(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz) as s:
+        s.set_kernel(kernel)
+        kname = binding.KERNEL_NAMES[s.get_kernel()]
+        out["kernel"] = kname
+        s.set_fraction(F_d, w.rho_l, w.rho_g)
+        s.sweeps(rhs_d, p_d, w.omega, min(fixed, 20))          # warm-up
+        torch.cuda.synchronize()
+        p_d.zero_()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record()
+        s.sweeps(rhs_d, p_d, w.omega, fixed)
+        ev1.record()
+        torch.cuda.synchronize()
+        ms = ev0.elapsed_time(ev1)
+        res = s.residual(rhs_d, p_d)
+        out.update(fixed_sweeps=fixed, fixed_ms=ms,
+                   gcell_per_s=w.cells * fixed / (ms / 1e3) / 1e9,
+                   model_gb_per_s=w.cells * fixed * BYTES_PER_UPDATE[kname] / (ms / 1e3) / 1e9,
+                   res_rel_after_fixed=res[1])
+        if to_tol:
+            p_d.zero_()
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            info = s.solve(rhs_d, p_d, w.omega, max_sweeps, 1e-8)
+            torch.cuda.synchronize()
+            out.update(tol_seconds=time.perf_counter() - t0, tol_sweeps=info.sweeps,
+                       tol_converged=bool(info.converged), tol_res_rel=info.res_rel)
+    return out
+
+
+def to_markdown(rows) -> str:
+    head = ("| cfg | workload | kernel | sweeps | ms | Gcell-upd/s | model GB/s | res_rel after | "
+            "to 1e-8: sweeps | seconds | res_rel |\n|---|---|---|---|---|---|---|---|---|---|---|\n")
+    body = ""
+    for r in rows:
+        tol = (f"{r['tol_sweeps']}{'' if r['tol_converged'] else ' (not converged)'} | "
+               f"{r['tol_seconds']:.2f} | {r['tol_res_rel']:.3e}") if "tol_sweeps" in r else "- | - | -"
+        body += (f"| {r['config']} | {r['workload']} | {r['kernel']} | {r['fixed_sweeps']} | "
+                 f"{r['fixed_ms']:.2f} | {r['gcell_per_s']:.1f} | {r['model_gb_per_s']:.0f} | "
+                 f"{r['res_rel_after_fixed']:.3e} | {tol} |\n")
+    return head + body
+
+
+def main(argv=None):
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--configs", default="1,2,3,4,5")
+    ap.add_argument("--max-sweeps", type=int, default=1_000_000)
+    ap.add_argument("--no-tol", action="store_true", help="skip the to-tolerance solves")
+    ap.add_argument("--kernel", default="auto", choices=["auto", "twopass", "fused"])
+    ap.add_argument("--md", default="", help="also write the table to this file")
+    args = ap.parse_args(argv)
+    import torch
+    from . import binding, build
+    if not torch.cuda.is_available():
+        raise SystemExit("report: no CUDA device (the CUDA path is the only path)")
+    build.build()
+    binding.load()
+    kernel = {"auto": binding.KERNEL_AUTO, "twopass": binding.KERNEL_TWOPASS,
+              "fused": binding.KERNEL_FUSED}[args.kernel]
+    rows = []
+    for cfg in [int(c) for c in args.configs.split(",")]:
+        r = run_config(cfg, args.max_sweeps, to_tol=(not args.no_tol and cfg != 5), kernel=kernel)
+        print(json.dumps(r), file=sys.stderr, flush=True)
+        rows.append(r)
+    md = to_markdown(rows)
+    print(md)
+    if args.md:
+        with open(args.md, "w") as f:
+            f.write(md)
+
+
+if __name__ == "__main__":
+    main()
