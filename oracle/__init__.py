@@ -148,3 +148,81 @@ def threads() -> int:
         return len(os.sched_getaffinity(0))
     except AttributeError:
         return os.cpu_count() or 1
+
+
+# ----------------------------------------------------------------------------- multigrid (M1-M6)
+class _MgParams(ctypes.Structure):
+    _fields_ = [("levels", ctypes.c_int), ("nu1", ctypes.c_int), ("nu2", ctypes.c_int),
+                ("coarse_sweeps", ctypes.c_int), ("gamma", ctypes.c_int),
+                ("omega_s", ctypes.c_double)]
+
+
+def _mg_lib():
+    lib = _load()
+    if not getattr(lib, "_mg_ready", False):
+        dp, i, d = ctypes.POINTER(ctypes.c_double), ctypes.c_int, ctypes.c_double
+        lib.ora_mg_coarsen.argtypes = [i, i, i, dp, dp, dp, dp, dp, dp]
+        lib.ora_mg_residual_field.argtypes = [i, i, i, dp, dp, dp, dp, dp, dp]
+        lib.ora_mg_restrict.argtypes = [i, i, i, dp, dp]
+        lib.ora_mg_prolong_add.argtypes = [i, i, i, dp, dp]
+        lib.ora_mg_max_levels.argtypes = [i, i, i]
+        lib.ora_mg_max_levels.restype = i
+        lib.ora_mg_solve.argtypes = [i, i, i, dp, dp, dp, dp, dp, ctypes.POINTER(_MgParams), i, d,
+                                     ctypes.POINTER(_Info)]
+        lib.ora_mg_solve.restype = i
+        for f in ("ora_mg_coarsen", "ora_mg_residual_field", "ora_mg_restrict",
+                  "ora_mg_prolong_add"):
+            getattr(lib, f).restype = None
+        lib._mg_ready = True
+    return lib
+
+
+def mg_coarsen(coef):
+    """M1: coarse (ax, ay, az) on the nx/2 x ny/2 x nz/2 grid."""
+    ax, ay, az = coef
+    nx, ny, nz = _shape(ax)
+    out = [np.empty((nz // 2, ny // 2, nx // 2)) for _ in range(3)]
+    _mg_lib().ora_mg_coarsen(nx, ny, nz, _p(ax), _p(ay), _p(az), _p(out[0]), _p(out[1]), _p(out[2]))
+    return tuple(out)
+
+
+def mg_residual_field(coef, rhs: np.ndarray, p: np.ndarray) -> np.ndarray:
+    """M2: r = rhs - A p."""
+    ax, ay, az = coef
+    nx, ny, nz = _shape(p)
+    r = np.empty_like(p)
+    _mg_lib().ora_mg_residual_field(nx, ny, nz, _p(ax), _p(ay), _p(az), _p(rhs), _p(p), _p(r))
+    return r
+
+
+def mg_restrict(r: np.ndarray) -> np.ndarray:
+    """M3: mean of the 8 children."""
+    nx, ny, nz = _shape(r)
+    rc = np.empty((nz // 2, ny // 2, nx // 2))
+    _mg_lib().ora_mg_restrict(nx, ny, nz, _p(r), _p(rc))
+    return rc
+
+
+def mg_prolong_add(ec: np.ndarray, p: np.ndarray) -> None:
+    """M4: p += piecewise-constant interpolation of ec (in place)."""
+    nx, ny, nz = _shape(p)
+    _mg_lib().ora_mg_prolong_add(nx, ny, nz, _p(ec), _p(p))
+
+
+def mg_max_levels(nx: int, ny: int, nz: int) -> int:
+    return _mg_lib().ora_mg_max_levels(nx, ny, nz)
+
+
+def mg_solve(coef, rhs: np.ndarray, p: np.ndarray, max_cycles: int, tol: float, levels: int = 99,
+             nu1: int = 2, nu2: int = 2, coarse_sweeps: int = 50, gamma: int = 1,
+             omega_s: float = 1.2) -> Info:
+    """M5 + M6 in place on p; Info.sweeps holds the number of cycles."""
+    ax, ay, az = coef
+    nx, ny, nz = _shape(p)
+    prm = _MgParams(levels, nu1, nu2, coarse_sweeps, gamma, omega_s)
+    info = _Info()
+    rc = _mg_lib().ora_mg_solve(nx, ny, nz, _p(ax), _p(ay), _p(az), _p(rhs), _p(p),
+                                ctypes.byref(prm), max_cycles, tol, ctypes.byref(info))
+    if rc != 0:
+        raise MemoryError("ora_mg_solve")
+    return Info(info.sweeps, bool(info.converged), info.res_abs, info.res_rel, info.rhs_norm)

@@ -174,3 +174,185 @@ void ora_solve(int nx, int ny, int nz, const double *ax, const double *ay, const
     info->res_rel = rr;
     info->rhs_norm = bn;
 }
+
+/* =====================================================================================
+ * Multigrid acceleration of the red-black SOR ("multigrid accelerated red black SOR
+ * relaxation scheme").  The paper gives no detail beyond those words, so
+ * every choice below is a reading listed in DESIGN.md §12 (M1-M6): geometric cell-centred
+ * coarsening by 2 in x, y and z, rediscretised coarse operator from averaged face coefficients,
+ * 8-cell averaging restriction, piecewise-constant prolongation, red-black SOR as smoother and
+ * as coarsest-level solver, V (gamma = 1) or W (gamma = 2) cycle.
+ * Pins (tests/test_oracle_mg_pins.py): constant-rho coarse operator = the fine formula at 2h;
+ * restriction/prolongation adjointness; coarse coefficients keep symmetry and zero row sums;
+ * two-level cycle with an exact coarse solve reproduces the dense two-grid operator; the
+ * converged result equals the dense LU solution; convergence factor of a constant-rho V-cycle.
+ * ===================================================================================== */
+
+/* M1: coarse face coefficient = 1/16 of the sum of the 4 fine face coefficients lying on the
+ * coarse face (their arithmetic mean, times h^2/H^2 = 1/4).  Fine grid nx x ny x nz (all even),
+ * coarse grid nx/2 x ny/2 x nz/2.  Wall faces stay 0 (the fine wall faces are 0), z wraps. */
+void ora_mg_coarsen(int nx, int ny, int nz, const double *ax, const double *ay, const double *az,
+                    double *axc, double *ayc, double *azc)
+{
+    const int cx = nx / 2, cy = ny / 2, cz = nz / 2;
+    for (int K = 0; K < cz; ++K)
+        for (int J = 0; J < cy; ++J)
+            for (int I = 0; I < cx; ++I) {
+                const size_t c = (size_t)I + (size_t)cx * ((size_t)J + (size_t)cy * (size_t)K);
+                const int i = 2 * I, j = 2 * J, k = 2 * K;
+                axc[c] = 0.0625 * (((ax[IDX(i + 1, j, k)] + ax[IDX(i + 1, j + 1, k)])
+                                    + ax[IDX(i + 1, j, k + 1)]) + ax[IDX(i + 1, j + 1, k + 1)]);
+                ayc[c] = 0.0625 * (((ay[IDX(i, j + 1, k)] + ay[IDX(i + 1, j + 1, k)])
+                                    + ay[IDX(i, j + 1, k + 1)]) + ay[IDX(i + 1, j + 1, k + 1)]);
+                azc[c] = 0.0625 * (((az[IDX(i, j, k + 1)] + az[IDX(i + 1, j, k + 1)])
+                                    + az[IDX(i, j + 1, k + 1)]) + az[IDX(i + 1, j + 1, k + 1)]);
+            }
+}
+
+/* M2: residual field r = rhs - A p (the same expression as O5, stored). */
+void ora_mg_residual_field(int nx, int ny, int nz, const double *ax, const double *ay,
+                           const double *az, const double *rhs, const double *p, double *r)
+{
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) {
+                double s, d;
+                stencil_sums(nx, ny, nz, ax, ay, az, p, i, j, k, &s, &d);
+                const size_t n = IDX(i, j, k);
+                r[n] = rhs[n] - (s - d * p[n]);
+            }
+}
+
+/* M3: restriction = mean of the 8 children, summed with x fastest, then y, then z. */
+void ora_mg_restrict(int nx, int ny, int nz, const double *r, double *rc)
+{
+    const int cx = nx / 2, cy = ny / 2, cz = nz / 2;
+    for (int K = 0; K < cz; ++K)
+        for (int J = 0; J < cy; ++J)
+            for (int I = 0; I < cx; ++I) {
+                const int i = 2 * I, j = 2 * J, k = 2 * K;
+                double t = r[IDX(i, j, k)] + r[IDX(i + 1, j, k)];
+                t = t + r[IDX(i, j + 1, k)];
+                t = t + r[IDX(i + 1, j + 1, k)];
+                t = t + r[IDX(i, j, k + 1)];
+                t = t + r[IDX(i + 1, j, k + 1)];
+                t = t + r[IDX(i, j + 1, k + 1)];
+                t = t + r[IDX(i + 1, j + 1, k + 1)];
+                rc[(size_t)I + (size_t)cx * ((size_t)J + (size_t)cy * (size_t)K)] = 0.125 * t;
+            }
+}
+
+/* M4: piecewise-constant prolongation, added to the fine iterate: p_c += e_parent(c). */
+void ora_mg_prolong_add(int nx, int ny, int nz, const double *ec, double *p)
+{
+    const int cx = nx / 2, cy = ny / 2;
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i)
+                p[IDX(i, j, k)] = p[IDX(i, j, k)]
+                    + ec[(size_t)(i / 2) + (size_t)cx * ((size_t)(j / 2) + (size_t)cy * (size_t)(k / 2))];
+}
+
+/* M5: number of levels the grid allows: coarsen while nx, ny are even with nx/2, ny/2 >= 2 and
+ * nz is a multiple of 4 (the coarse nz must stay even for the red-black colouring across the
+ * periodic wrap). */
+int ora_mg_max_levels(int nx, int ny, int nz)
+{
+    int L = 1;
+    while (nx % 2 == 0 && ny % 2 == 0 && nz % 4 == 0 && nx / 2 >= 2 && ny / 2 >= 2) {
+        nx /= 2; ny /= 2; nz /= 2; ++L;
+    }
+    return L;
+}
+
+typedef struct {
+    int nx, ny, nz;
+    double *ax, *ay, *az;   /* level 0: the caller's arrays */
+    double *rhs, *p, *r;    /* level 0: rhs and p are the caller's */
+} mg_level;
+
+#include <stdlib.h>
+#include <string.h>
+
+/* M6: one cycle on level l.  Coarsest level: coarse_sweeps SOR sweeps.  Otherwise nu1 sweeps,
+ * residual, restriction to the rhs of level l+1, zero initial guess there, gamma recursive
+ * cycles (1 = V, 2 = W), prolongation added to p, nu2 sweeps. */
+static void mg_cycle(mg_level *lv, int l, int nlev, const ora_mg_params *prm)
+{
+    mg_level *f = &lv[l];
+    if (l == nlev - 1) {
+        for (int s = 0; s < prm->coarse_sweeps; ++s)
+            ora_sweep(f->nx, f->ny, f->nz, f->ax, f->ay, f->az, f->rhs, f->p, prm->omega_s);
+        return;
+    }
+    mg_level *c = &lv[l + 1];
+    for (int s = 0; s < prm->nu1; ++s)
+        ora_sweep(f->nx, f->ny, f->nz, f->ax, f->ay, f->az, f->rhs, f->p, prm->omega_s);
+    ora_mg_residual_field(f->nx, f->ny, f->nz, f->ax, f->ay, f->az, f->rhs, f->p, f->r);
+    ora_mg_restrict(f->nx, f->ny, f->nz, f->r, c->rhs);
+    memset(c->p, 0, sizeof(double) * (size_t)c->nx * c->ny * c->nz);
+    for (int g = 0; g < prm->gamma; ++g) mg_cycle(lv, l + 1, nlev, prm);
+    ora_mg_prolong_add(f->nx, f->ny, f->nz, c->p, f->p);
+    for (int s = 0; s < prm->nu2; ++s)
+        ora_sweep(f->nx, f->ny, f->nz, f->ax, f->ay, f->az, f->rhs, f->p, prm->omega_s);
+}
+
+/* Multigrid solve: cycles c = 1..max_cycles from the caller's p, the O5 norm after every cycle,
+ * stop at the first cycle with ||r||/||rhs|| <= tol (tol <= 0: exactly max_cycles cycles).
+ * prm->levels is clipped to [1, ora_mg_max_levels].  info->sweeps returns the cycles done.
+ * Returns 0, or -1 if memory ran out. */
+int ora_mg_solve(int nx, int ny, int nz, const double *ax, const double *ay, const double *az,
+                 const double *rhs, double *p, const ora_mg_params *prm, int max_cycles,
+                 double tol, ora_info *info)
+{
+    int nlev = prm->levels, maxl = ora_mg_max_levels(nx, ny, nz);
+    if (nlev > maxl) nlev = maxl;
+    if (nlev < 1) nlev = 1;
+    mg_level lv[32];
+    memset(lv, 0, sizeof lv);
+    lv[0].nx = nx; lv[0].ny = ny; lv[0].nz = nz;
+    lv[0].ax = (double *)ax; lv[0].ay = (double *)ay; lv[0].az = (double *)az;
+    lv[0].rhs = (double *)rhs; lv[0].p = p;
+    int ok = 1;
+    for (int l = 0; l < nlev && ok; ++l) {
+        const size_t n = (size_t)lv[l].nx * lv[l].ny * lv[l].nz;
+        lv[l].r = (double *)malloc(n * sizeof(double));
+        ok = ok && lv[l].r;
+        if (l > 0) {
+            lv[l].ax = (double *)malloc(n * sizeof(double));
+            lv[l].ay = (double *)malloc(n * sizeof(double));
+            lv[l].az = (double *)malloc(n * sizeof(double));
+            lv[l].rhs = (double *)malloc(n * sizeof(double));
+            lv[l].p = (double *)malloc(n * sizeof(double));
+            ok = ok && lv[l].ax && lv[l].ay && lv[l].az && lv[l].rhs && lv[l].p;
+            if (ok)
+                ora_mg_coarsen(lv[l - 1].nx, lv[l - 1].ny, lv[l - 1].nz, lv[l - 1].ax, lv[l - 1].ay,
+                               lv[l - 1].az, lv[l].ax, lv[l].ay, lv[l].az);
+        }
+        if (l + 1 < nlev) {
+            lv[l + 1].nx = lv[l].nx / 2; lv[l + 1].ny = lv[l].ny / 2; lv[l + 1].nz = lv[l].nz / 2;
+        }
+    }
+    double ra = 0.0, rr = 0.0, bn = 0.0;
+    int c = 0, converged = 0;
+    if (ok) {
+        for (c = 1; c <= max_cycles; ++c) {
+            mg_cycle(lv, 0, nlev, prm);
+            ora_residual(nx, ny, nz, ax, ay, az, rhs, p, &ra, &rr, &bn);
+            if (tol > 0.0 && rr <= tol) { converged = 1; break; }
+        }
+        if (c > max_cycles) c = max_cycles;
+        if (max_cycles == 0) ora_residual(nx, ny, nz, ax, ay, az, rhs, p, &ra, &rr, &bn);
+    }
+    for (int l = 0; l < nlev; ++l) {
+        free(lv[l].r);
+        if (l > 0) { free(lv[l].ax); free(lv[l].ay); free(lv[l].az); free(lv[l].rhs); free(lv[l].p); }
+    }
+    if (!ok) return -1;
+    info->sweeps = c;
+    info->converged = converged;
+    info->res_abs = ra;
+    info->res_rel = rr;
+    info->rhs_norm = bn;
+    return 0;
+}

@@ -31,6 +31,26 @@ void ora_solve(int nx, int ny, int nz, const double *ax, const double *ay, const
                const double *rhs, double *p, double omega, int max_sweeps, double tol,
                int check_interval, ora_info *info);
 
+/* Multigrid acceleration (readings M1-M6 of DESIGN.md §12). */
+typedef struct {
+    int levels;          /* requested number of levels (clipped to what the grid allows) */
+    int nu1, nu2;        /* pre- and post-smoothing sweeps */
+    int coarse_sweeps;   /* SOR sweeps on the coarsest level */
+    int gamma;           /* recursive cycles per level: 1 = V, 2 = W */
+    double omega_s;      /* relaxation factor of the smoother and coarsest solver */
+} ora_mg_params;
+
+void ora_mg_coarsen(int nx, int ny, int nz, const double *ax, const double *ay, const double *az,
+                    double *axc, double *ayc, double *azc);
+void ora_mg_residual_field(int nx, int ny, int nz, const double *ax, const double *ay,
+                           const double *az, const double *rhs, const double *p, double *r);
+void ora_mg_restrict(int nx, int ny, int nz, const double *r, double *rc);
+void ora_mg_prolong_add(int nx, int ny, int nz, const double *ec, double *p);
+int ora_mg_max_levels(int nx, int ny, int nz);
+int ora_mg_solve(int nx, int ny, int nz, const double *ax, const double *ay, const double *az,
+                 const double *rhs, double *p, const ora_mg_params *prm, int max_cycles,
+                 double tol, ora_info *info);
+
 #ifdef __cplusplus
 }
 #endif

@@ -1,0 +1,166 @@
+"""Pins of the oracle's multigrid steps M1-M6 ("multigrid accelerated red black SOR";
+readings in DESIGN.md §12).  The paper gives no multigrid detail, so the pins are what the
+mathematics fixes: the coarse operator of a constant-density problem is the fine formula at 2h,
+the Galerkin relation R A P = 2 A_c that ties coarsening, restriction and prolongation to the
+(already pinned) fine operator, adjointness of R and P, symmetry and zero row sums of every
+coarse operator, reduction to plain SOR with one level, convergence to the dense LU solution,
+and textbook convergence behaviour of a constant-coefficient V-cycle.
+"""
+import numpy as np
+import pytest
+
+from paper_2104_01636_b200 import workload as wl
+
+
+def rnd(shape, seed, stream=9):
+    n = int(np.prod(shape))
+    return (2.0 * wl.uniform01(seed, stream, np.arange(n, dtype=np.uint64)) - 1.0).reshape(shape)
+
+
+def var_coef(ora, nx, ny, nz, seed, h=(0.1, 0.07, 0.13)):
+    F = wl.random_fraction(nx, ny, nz, seed)
+    return ora.coefficients(F, 1000.0, 1.2, *h)
+
+
+# ------------------------------------------------------------------ M1
+@pytest.mark.parametrize("Fval", [1.0, 0.25])
+def test_coarse_operator_of_constant_density_is_the_2h_formula(ora, Fval):
+    nx, ny, nz, dx, dy, dz = 8, 12, 16, 0.1, 0.07, 0.13
+    fine = ora.coefficients(np.full((nz, ny, nx), Fval), 1000.0, 1.2, dx, dy, dz)
+    want = ora.coefficients(np.full((nz // 2, ny // 2, nx // 2), Fval), 1000.0, 1.2,
+                            2 * dx, 2 * dy, 2 * dz)
+    got = ora.mg_coarsen(fine)
+    for g, w in zip(got, want):
+        assert np.max(np.abs(g - w)) <= 4e-16 * np.max(np.abs(w))
+    assert np.all(got[0][:, :, -1] == 0.0) and np.all(got[1][:, -1, :] == 0.0)   # walls stay closed
+    assert np.all(got[2] > 0.0)                                                   # z wraps
+
+
+def test_galerkin_relation_ties_transfer_and_coarsening_to_the_fine_operator(ora):
+    """For a coarse field E: restrict(A_f prolong(E)) = 2 A_c E  (fluxes through the 4 fine faces
+    of every coarse face add up; R = 1/8 sum, a_F = 1/16 sum).  A wrong face index, weight or
+    child order in M1, M3 or M4 breaks it."""
+    nx, ny, nz = 8, 6, 12
+    fine = var_coef(ora, nx, ny, nz, 3)
+    coarse = ora.mg_coarsen(fine)
+    E = rnd((nz // 2, ny // 2, nx // 2), 5)
+    PE = np.zeros((nz, ny, nx))
+    ora.mg_prolong_add(E, PE)
+    lhs = ora.mg_restrict(ora.apply(fine, PE))
+    rhs = 2.0 * ora.apply(coarse, E)
+    assert np.max(np.abs(lhs - rhs)) <= 1e-13 * np.max(np.abs(rhs))
+
+
+def test_coarse_operators_stay_symmetric_with_zero_row_sums(ora):
+    coef = var_coef(ora, 16, 8, 16, 11)
+    for _ in range(2):
+        coef = ora.mg_coarsen(coef)
+        shape = coef[0].shape
+        x, y = rnd(shape, 1), rnd(shape, 2)
+        a, b = float(np.sum(x * ora.apply(coef, y))), float(np.sum(y * ora.apply(coef, x)))
+        assert abs(a - b) <= 1e-13 * max(abs(a), abs(b))
+        ones = ora.apply(coef, np.ones(shape))
+        assert np.max(np.abs(ones)) <= 1e-12 * np.max(coef[2])
+
+
+# ------------------------------------------------------------------ M2
+def test_residual_field_is_rhs_minus_apply_and_matches_the_norm(ora):
+    nx, ny, nz = 10, 6, 8
+    coef = var_coef(ora, nx, ny, nz, 4)
+    rhs, p = rnd((nz, ny, nx), 6), rnd((nz, ny, nx), 7)
+    r = ora.mg_residual_field(coef, rhs, p)
+    assert np.max(np.abs(r - (rhs - ora.apply(coef, p)))) <= 1e-12 * np.max(np.abs(r))
+    res_abs = ora.residual(coef, rhs, p)[0]
+    assert abs(np.linalg.norm(r) - res_abs) <= 1e-13 * res_abs
+
+
+# ------------------------------------------------------------------ M3, M4
+def test_transfer_operators_constants_sums_and_adjointness(ora):
+    nx, ny, nz = 6, 10, 8
+    r = rnd((nz, ny, nx), 8)
+    rc = ora.mg_restrict(r)
+    assert rc.shape == (nz // 2, ny // 2, nx // 2)
+    assert abs(8.0 * rc.sum() - r.sum()) <= 1e-13 * np.abs(r).sum()
+    assert np.all(ora.mg_restrict(np.full((nz, ny, nx), 3.5)) == 3.5)
+    p = np.full((nz, ny, nx), 1.0)
+    ora.mg_prolong_add(np.full(rc.shape, 2.0), p)
+    assert np.all(p == 3.0)
+    e = rnd(rc.shape, 9)
+    Pe = np.zeros((nz, ny, nx))
+    ora.mg_prolong_add(e, Pe)
+    assert abs(8.0 * np.sum(rc * e) - np.sum(r * Pe)) <= 1e-13 * np.sum(np.abs(r * Pe))
+    # a single coarse value lands on exactly its 8 children
+    e1 = np.zeros(rc.shape)
+    e1[1, 2, 1] = 1.0
+    P1 = np.zeros((nz, ny, nx))
+    ora.mg_prolong_add(e1, P1)
+    assert P1.sum() == 8.0 and np.all(P1[2:4, 4:6, 2:4] == 1.0)
+
+
+# ------------------------------------------------------------------ M5
+def test_level_count_rule(ora):
+    assert ora.mg_max_levels(256, 256, 512) == 8       # 2x2x4 at the bottom
+    assert ora.mg_max_levels(32, 32, 64) == 5
+    assert ora.mg_max_levels(16, 12, 20) == 2          # nz = 20 -> 10 (even), then 10 % 4 != 0
+    assert ora.mg_max_levels(5, 7, 6) == 1
+    assert ora.mg_max_levels(4, 4, 6) == 1             # coarse nz would be odd
+
+
+# ------------------------------------------------------------------ M6
+def test_one_level_cycle_is_plain_sor(ora):
+    nx, ny, nz = 8, 8, 8
+    coef = var_coef(ora, nx, ny, nz, 12)
+    rhs = wl.remove_mean(rnd((nz, ny, nx), 13))
+    p1, p2 = np.zeros_like(rhs), np.zeros_like(rhs)
+    ora.mg_solve(coef, rhs, p1, 3, 0.0, levels=1, coarse_sweeps=7, omega_s=1.3)
+    ora.sweep(coef, rhs, p2, 1.3, 21)
+    assert np.array_equal(p1, p2)
+
+
+@pytest.mark.parametrize("gamma", [1, 2])
+def test_mg_converges_to_the_dense_lu_solution(ora, gamma):
+    nx, ny, nz = 4, 4, 8
+    N = nx * ny * nz
+    coef = var_coef(ora, nx, ny, nz, 21, h=(0.25, 0.25, 0.125))
+    rhs = wl.remove_mean(rnd((nz, ny, nx), 22))
+    A = np.empty((N, N))
+    for n in range(N):                                   # columns of A through the pinned operator
+        e = np.zeros(N)
+        e[n] = 1.0
+        A[:, n] = ora.apply(coef, e.reshape(nz, ny, nx)).reshape(-1)
+    x = np.linalg.solve(A - np.ones((N, N)) / N, rhs.reshape(-1))
+    p = np.zeros_like(rhs)
+    info = ora.mg_solve(coef, rhs, p, 200, 1e-13, levels=2, nu1=2, nu2=2, coarse_sweeps=60,
+                        gamma=gamma, omega_s=1.2)
+    assert info.converged and info.res_rel <= 1e-13
+    q = p.reshape(-1) - p.mean()
+    assert np.max(np.abs(q - (x - x.mean()))) <= 1e-10 * np.max(np.abs(x))
+
+
+def test_constant_density_v_cycle_converges_at_a_grid_independent_rate(ora):
+    """Textbook multigrid behaviour: with constant coefficients the residual reduction per V(2,2)
+    cycle is bounded well below 1 and does not degrade when the grid is refined (plain SOR's
+    rate tends to 1 like 1 - O(h^2))."""
+    factors = []
+    for nx, ny, nz in ((16, 16, 32), (32, 32, 64)):
+        coef = ora.coefficients(np.ones((nz, ny, nx)), 1000.0, 1.2, 1 / nx, 1 / nx, 1 / nx)
+        rhs = wl.remove_mean(rnd((nz, ny, nx), 31))
+        p = np.zeros_like(rhs)
+        res = [1.0]
+        for _ in range(8):
+            res.append(ora.mg_solve(coef, rhs, p, 1, 0.0, levels=99, nu1=2, nu2=2,
+                                    coarse_sweeps=30, gamma=1, omega_s=1.0).res_rel)
+        assert all(b < a for a, b in zip(res, res[1:]))
+        factors.append((res[-1] / res[3]) ** (1.0 / 5))
+    assert max(factors) < 0.5
+    assert factors[1] < factors[0] * 1.25
+
+
+def test_mg_needs_far_fewer_passes_than_sor_on_a_bubbly_duct(ora):
+    w = wl.make_custom(32, 32, 64, 2, 8, 7)
+    coef = ora.coefficients(w.F, w.rho_l, w.rho_g, w.dx, w.dy, w.dz)
+    p = np.zeros_like(w.rhs)
+    info = ora.mg_solve(coef, w.rhs, p, 60, 1e-8, levels=3, nu1=2, nu2=2, coarse_sweeps=200,
+                        gamma=1, omega_s=1.2)
+    assert info.converged and info.sweeps <= 60       # plain SOR: thousands of sweeps (config 1)
+    assert abs(ora.residual(coef, w.rhs, p)[1] - info.res_rel) <= 1e-12 * info.res_rel
