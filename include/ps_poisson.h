@@ -148,6 +148,43 @@ int ps_solve_host(ps_ctx *c, const double *F_host, double rho_l, double rho_g,
 int ps_enable_timing(ps_ctx *c, int on);
 int ps_timing(ps_ctx *c, double *sweep_ms, long long *sweep_launches);
 
+/* ------------------------------------------------------------------------------------------
+ * Multigrid acceleration of the red-black SOR ("multigrid accelerated red black SOR
+ * relaxation scheme implemented on a GPU").  The paper gives no further
+ * detail; DESIGN.md §12 lists the readings M1-M6: geometric coarsening by 2 in x, y, z while nx,
+ * ny stay even and >= 2 after halving and nz is a multiple of 4; coarse face coefficient =
+ * 1/16 of the sum of the 4 fine face coefficients on the coarse face; restriction = mean of the
+ * 8 children of r = rhs - A p; piecewise-constant prolongation added to p; red-black SOR
+ * (omega_s) as smoother (nu1 before, nu2 after) and as coarsest-level solver (coarse_sweeps);
+ * gamma = 1 (V cycle) or 2 (W cycle). */
+typedef struct {
+    int levels;          /* requested levels, clipped to [1, what the grid allows]            */
+    int nu1, nu2;        /* pre-/post-smoothing sweeps (>= 0)                                  */
+    int coarse_sweeps;   /* sweeps on the coarsest level (>= 1)                                */
+    int gamma;           /* 1 = V, 2 = W                                                       */
+    double omega_s;      /* relaxation factor of smoother and coarsest solver, in (0,2)        */
+} ps_mg_params;
+
+/* Build the level hierarchy from the coefficients of the last ps_set_fraction (one coarsening
+ * launch per level; device memory for the levels is allocated by the library and freed by
+ * ps_destroy or the next ps_mg_setup).  Must be called again after every ps_set_fraction.
+ * PS_EINVAL: bad parameters.  PS_ESTATE: no coefficients. */
+int ps_mg_setup(ps_ctx *c, const ps_mg_params *prm);
+int ps_mg_levels(const ps_ctx *c);           /* levels in use (0 before ps_mg_setup) */
+
+/* Multigrid cycles c = 1..max_cycles from the caller's p (in/out); after every cycle the
+ * deterministic norm of ps_residual; stops at the first cycle with ||r||_2/||rhs||_2 <= tol
+ * (tol <= 0: exactly max_cycles cycles).  info->sweeps returns the number of cycles.
+ * Synchronises the stream once per cycle (the norm read-back).  PS_ESTATE without ps_mg_setup. */
+int ps_mg_solve(ps_ctx *c, const double *rhs_dev, double *p_dev, int max_cycles, double tol,
+                ps_info *info);
+
+/* The transfer operators on their own (parity tests): coarse coefficients of level 1 copied
+ * out (nx/2 * ny/2 * nz/2 doubles each, any may be NULL); rc = restriction of rhs - A p. */
+int ps_mg_export_coarse(ps_ctx *c, int level, double *ax_dev, double *ay_dev, double *az_dev);
+int ps_mg_residual_restrict(ps_ctx *c, const double *rhs_dev, const double *p_dev, double *rc_dev);
+int ps_mg_prolong_add(ps_ctx *c, const double *ec_dev, double *p_dev);
+
 /* Kernels launched by this context since ps_create (bench.py's gpu_launches). */
 long long ps_launch_count(const ps_ctx *c);
 

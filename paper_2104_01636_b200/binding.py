@@ -25,13 +25,21 @@ SYMBOLS = ("ps_create", "ps_destroy", "ps_workspace_bytes", "ps_set_workspace", 
            "ps_set_check_interval", "ps_set_kernel", "ps_get_kernel", "ps_set_tuning",
            "ps_get_tuning", "ps_set_fraction",
            "ps_export_coefficients", "ps_solve", "ps_sweeps", "ps_half_sweep", "ps_residual",
-           "ps_solve_host", "ps_enable_timing", "ps_timing", "ps_launch_count", "ps_strerror")
+           "ps_solve_host", "ps_enable_timing", "ps_timing", "ps_launch_count", "ps_strerror",
+           "ps_mg_setup", "ps_mg_levels", "ps_mg_solve", "ps_mg_export_coarse",
+           "ps_mg_residual_restrict", "ps_mg_prolong_add")
 
 
 class PsError(RuntimeError):
     def __init__(self, code: int, msg: str):
         super().__init__(f"libps_poisson: {msg} (code {code})")
         self.code = code
+
+
+class _MgParams(ctypes.Structure):
+    _fields_ = [("levels", ctypes.c_int), ("nu1", ctypes.c_int), ("nu2", ctypes.c_int),
+                ("coarse_sweeps", ctypes.c_int), ("gamma", ctypes.c_int),
+                ("omega_s", ctypes.c_double)]
 
 
 class _Info(ctypes.Structure):
@@ -86,6 +94,12 @@ def load(path: str | None = None) -> ctypes.CDLL:
     lib.ps_timing.argtypes = [vp, dp, ctypes.POINTER(ctypes.c_longlong)]
     lib.ps_launch_count.argtypes = [vp]
     lib.ps_launch_count.restype = ctypes.c_longlong
+    lib.ps_mg_setup.argtypes = [vp, ctypes.POINTER(_MgParams)]
+    lib.ps_mg_levels.argtypes = [vp]
+    lib.ps_mg_solve.argtypes = [vp, vp, vp, i, d, ctypes.POINTER(_Info)]
+    lib.ps_mg_export_coarse.argtypes = [vp, i, vp, vp, vp]
+    lib.ps_mg_residual_restrict.argtypes = [vp, vp, vp, vp]
+    lib.ps_mg_prolong_add.argtypes = [vp, vp, vp]
     lib.ps_strerror.argtypes = [i]
     lib.ps_strerror.restype = ctypes.c_char_p
     if path == _build.LIB:
@@ -236,6 +250,51 @@ class PoissonSolver:
                                                 _dev_ptr(p, self.shape, "p"), ctypes.byref(ra),
                                                 ctypes.byref(rr), ctypes.byref(bn)))
         return ra.value, rr.value, bn.value
+
+    # -- multigrid acceleration
+    def mg_setup(self, levels: int = 99, nu1: int = 2, nu2: int = 2, coarse_sweeps: int = 50,
+                 gamma: int = 1, omega_s: float = 1.2) -> int:
+        """Build the level hierarchy from the current coefficients; returns the levels in use."""
+        self._sync_stream()
+        prm = _MgParams(levels, nu1, nu2, coarse_sweeps, gamma, omega_s)
+        _check(self._lib, self._lib.ps_mg_setup(self._h, ctypes.byref(prm)))
+        return self._lib.ps_mg_levels(self._h)
+
+    def mg_solve(self, rhs, p, max_cycles: int, tol: float) -> Info:
+        """Multigrid cycles in place on p; Info.sweeps holds the number of cycles."""
+        self._sync_stream()
+        info = _Info()
+        _check(self._lib, self._lib.ps_mg_solve(self._h, _dev_ptr(rhs, self.shape, "rhs"),
+                                                _dev_ptr(p, self.shape, "p"), max_cycles, tol,
+                                                ctypes.byref(info)))
+        return Info(info.sweeps, bool(info.converged), info.res_abs, info.res_rel, info.rhs_norm)
+
+    def _coarse_shape(self, level: int = 1):
+        nz, ny, nx = self.shape
+        return (nz >> level, ny >> level, nx >> level)
+
+    def mg_export_coarse(self, level: int = 1):
+        import torch
+        self._sync_stream()
+        out = [torch.empty(self._coarse_shape(level), dtype=torch.float64, device="cuda")
+               for _ in range(3)]
+        _check(self._lib, self._lib.ps_mg_export_coarse(
+            self._h, level, *[ctypes.c_void_p(t.data_ptr()) for t in out]))
+        return tuple(out)
+
+    def mg_residual_restrict(self, rhs, p):
+        import torch
+        self._sync_stream()
+        rc = torch.empty(self._coarse_shape(1), dtype=torch.float64, device="cuda")
+        _check(self._lib, self._lib.ps_mg_residual_restrict(
+            self._h, _dev_ptr(rhs, self.shape, "rhs"), _dev_ptr(p, self.shape, "p"),
+            ctypes.c_void_p(rc.data_ptr())))
+        return rc
+
+    def mg_prolong_add(self, ec, p):
+        self._sync_stream()
+        _check(self._lib, self._lib.ps_mg_prolong_add(
+            self._h, _dev_ptr(ec, self._coarse_shape(1), "ec"), _dev_ptr(p, self.shape, "p")))
 
     def solve_host(self, F, rho_l: float, rho_g: float, rhs, p, omega: float, max_sweeps: int,
                    tol: float) -> Info:

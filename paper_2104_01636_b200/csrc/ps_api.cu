@@ -13,6 +13,7 @@
 #include "../../include/ps_poisson.h"
 #include "ps_kernels_generic.cuh"
 #include "ps_kernels_zmarch.cuh"
+#include "ps_kernels_mg.cuh"
 
 namespace {
 
@@ -60,6 +61,13 @@ struct ps_ctx {
     std::vector<cudaEvent_t> *ev;      // pairs: start, stop
     size_t ev_used;
     long long timed_launches;
+    // multigrid: the next coarser level is a context of its own; lv_rhs / lv_p are the right-hand
+    // side and the correction of THIS level when it is a coarse one (owned, cudaMalloc)
+    ps_ctx *child;
+    double *lv_rhs, *lv_p;
+    ps_mg_params mgp;
+    int mg_nlev;           // levels in use below and including this one (0: no hierarchy)
+    bool mg_ready;         // hierarchy matches the current coefficients
 };
 
 namespace {
@@ -241,6 +249,9 @@ int ps_create(ps_ctx **out, int nx, int ny, int nz, double dx, double dy, double
 int ps_destroy(ps_ctx *c)
 {
     if (!c) return PS_OK;
+    if (c->child) ps_destroy(c->child);
+    if (c->lv_rhs) cudaFree(c->lv_rhs);
+    if (c->lv_p) cudaFree(c->lv_p);
     if (c->ws && c->ws_owned) cudaFree(c->ws);
     if (c->h_scal) cudaFreeHost(c->h_scal);
     ps::zm_plan_destroy(&c->fused);
@@ -331,6 +342,7 @@ int ps_set_fraction(ps_ctx *c, const double *F_dev, double rho_l, double rho_g)
     c->launches++;
     PS_CUDA(cudaGetLastError());
     c->have_coef = true;
+    c->mg_ready = false;
     return PS_OK;
 }
 
@@ -470,7 +482,176 @@ int ps_timing(ps_ctx *c, double *sweep_ms, long long *sweep_launches)
     return PS_OK;
 }
 
-long long ps_launch_count(const ps_ctx *c) { return c ? c->launches : 0; }
+long long ps_launch_count(const ps_ctx *c)
+{
+    long long n = 0;
+    for (; c; c = c->child) n += c->launches;
+    return n;
+}
+
+}  // extern "C"
+
+// ----------------------------------------------------------------------------- multigrid
+namespace {
+
+int mg_max_levels(int nx, int ny, int nz)
+{
+    int L = 1;
+    while (nx % 2 == 0 && ny % 2 == 0 && nz % 4 == 0 && nx / 2 >= 2 && ny / 2 >= 2) {
+        nx /= 2; ny /= 2; nz /= 2; ++L;
+    }
+    return L;
+}
+
+int mg_launch_coarsen(ps_ctx *f, ps_ctx *k)
+{
+    ps::ps_mg_coarsen_kernel<<<grid_for(f, k->g.cells(), 256), 256, 0, f->stream>>>(
+        f->g, f->ax, f->ay, f->az, k->ax, k->ay, k->az);
+    f->launches++;
+    PS_CUDA(cudaGetLastError());
+    k->have_coef = true;
+    return PS_OK;
+}
+
+int mg_launch_residual_restrict(ps_ctx *f, const double *rhs, const double *p, double *rc)
+{
+    ps::ps_mg_residual_restrict_kernel<<<grid_for(f, f->g.cells() / 8, 256), 256, 0, f->stream>>>(
+        f->g, f->ax, f->ay, f->az, rhs, p, rc);
+    f->launches++;
+    PS_CUDA(cudaGetLastError());
+    return PS_OK;
+}
+
+int mg_launch_prolong_add(ps_ctx *f, const double *ec, double *p)
+{
+    ps::ps_mg_prolong_add_kernel<<<grid_for(f, f->g.cells() / 2, 256), 256, 0, f->stream>>>(
+        f->g, ec, p);
+    f->launches++;
+    PS_CUDA(cudaGetLastError());
+    return PS_OK;
+}
+
+// M6: one cycle on the level of context f.
+int mg_cycle(ps_ctx *f, const ps_mg_params &m, const double *rhs, double *p)
+{
+    int rc;
+    if (!f->child || f->mg_nlev <= 1)
+        return run_sweeps(f, rhs, p, m.omega_s, m.coarse_sweeps);
+    ps_ctx *k = f->child;
+    if ((rc = run_sweeps(f, rhs, p, m.omega_s, m.nu1))) return rc;
+    if ((rc = mg_launch_residual_restrict(f, rhs, p, k->lv_rhs))) return rc;
+    PS_CUDA(cudaMemsetAsync(k->lv_p, 0, k->g.cells() * sizeof(double), f->stream));
+    for (int g = 0; g < m.gamma; ++g)
+        if ((rc = mg_cycle(k, m, k->lv_rhs, k->lv_p))) return rc;
+    if ((rc = mg_launch_prolong_add(f, k->lv_p, p))) return rc;
+    return run_sweeps(f, rhs, p, m.omega_s, m.nu2);
+}
+
+}  // namespace
+
+extern "C" {
+
+int ps_mg_setup(ps_ctx *c, const ps_mg_params *prm)
+{
+    if (!c || !prm) return PS_EINVAL;
+    if (prm->nu1 < 0 || prm->nu2 < 0 || prm->coarse_sweeps < 1 || prm->gamma < 1 ||
+        prm->gamma > 2 || !(prm->omega_s > 0.0 && prm->omega_s < 2.0))
+        return PS_EINVAL;
+    if (!c->have_coef) return PS_ESTATE;
+    int nlev = prm->levels;
+    const int maxl = mg_max_levels(c->g.nx, c->g.ny, c->g.nz);
+    if (nlev > maxl) nlev = maxl;
+    if (nlev < 1) nlev = 1;
+    if (c->mg_nlev != nlev && c->child) {          // different depth: rebuild the chain
+        ps_destroy(c->child);
+        c->child = nullptr;
+    }
+    ps_ctx *f = c;
+    for (int l = 0; l < nlev; ++l) {
+        f->mg_nlev = nlev - l;
+        f->mgp = *prm;
+        if (l == nlev - 1) break;
+        if (!f->child) {
+            ps_ctx *k = nullptr;
+            int rc = ps_create(&k, f->g.nx / 2, f->g.ny / 2, f->g.nz / 2, 2.0 * f->dx, 2.0 * f->dy,
+                               2.0 * f->dz);
+            if (rc) return rc;
+            f->child = k;
+            if ((rc = ensure_workspace(k))) return rc;
+            const size_t b = k->g.cells() * sizeof(double);
+            cudaError_t e = cudaMalloc((void **)&k->lv_rhs, b);
+            if (e == cudaSuccess) e = cudaMalloc((void **)&k->lv_p, b);
+            if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); return PS_ENOMEM; }
+            if (e != cudaSuccess) return cuda_fail(e);
+        }
+        f->child->stream = c->stream;
+        const int rc = mg_launch_coarsen(f, f->child);
+        if (rc) return rc;
+        f = f->child;
+    }
+    c->mg_ready = true;
+    return PS_OK;
+}
+
+int ps_mg_levels(const ps_ctx *c) { return c ? c->mg_nlev : 0; }
+
+int ps_mg_solve(ps_ctx *c, const double *rhs_dev, double *p_dev, int max_cycles, double tol,
+                ps_info *info)
+{
+    if (!c || !rhs_dev || !p_dev || max_cycles < 0) return PS_EINVAL;
+    if (!c->have_coef || !c->mg_ready) return PS_ESTATE;
+    for (ps_ctx *k = c->child; k; k = k->child) k->stream = c->stream;
+    int cyc = 0, converged = 0, rc = 0;
+    for (cyc = 1; cyc <= max_cycles; ++cyc) {
+        if ((rc = mg_cycle(c, c->mgp, rhs_dev, p_dev))) return rc;
+        if ((rc = enqueue_residual(c, rhs_dev, p_dev, tol))) return rc;
+        PS_CUDA(cudaStreamSynchronize(c->stream));
+        if (tol > 0.0 && c->h_scal[1] <= tol) { converged = 1; break; }
+    }
+    if (cyc > max_cycles) cyc = max_cycles;
+    if (max_cycles == 0) {
+        if ((rc = enqueue_residual(c, rhs_dev, p_dev, tol))) return rc;
+        PS_CUDA(cudaStreamSynchronize(c->stream));
+    }
+    if (info) {
+        info->sweeps = cyc;
+        info->converged = converged;
+        info->res_abs = c->h_scal[0];
+        info->res_rel = c->h_scal[1];
+        info->rhs_norm = c->h_scal[2];
+    }
+    return PS_OK;
+}
+
+int ps_mg_export_coarse(ps_ctx *c, int level, double *ax_dev, double *ay_dev, double *az_dev)
+{
+    if (!c || level < 0) return PS_EINVAL;
+    if (!c->mg_ready) return PS_ESTATE;
+    if (level >= c->mg_nlev) return PS_EINVAL;
+    ps_ctx *k = c;
+    for (int l = 0; l < level; ++l) k = k->child;
+    k->stream = c->stream;
+    return ps_export_coefficients(k, ax_dev, ay_dev, az_dev);
+}
+
+int ps_mg_residual_restrict(ps_ctx *c, const double *rhs_dev, const double *p_dev, double *rc_dev)
+{
+    if (!c || !rhs_dev || !p_dev || !rc_dev) return PS_EINVAL;
+    if (!c->have_coef) return PS_ESTATE;
+    if (c->g.nx % 2 || c->g.ny % 2 || c->g.nz % 2) return PS_EINVAL;
+    return mg_launch_residual_restrict(c, rhs_dev, p_dev, rc_dev);
+}
+
+int ps_mg_prolong_add(ps_ctx *c, const double *ec_dev, double *p_dev)
+{
+    if (!c || !ec_dev || !p_dev) return PS_EINVAL;
+    if (c->g.nx % 2 || c->g.ny % 2 || c->g.nz % 2) return PS_EINVAL;
+    return mg_launch_prolong_add(c, ec_dev, p_dev);
+}
+
+}  // extern "C"
+
+extern "C" {
 
 const char *ps_strerror(int code)
 {

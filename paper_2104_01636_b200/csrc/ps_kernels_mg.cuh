@@ -1,0 +1,105 @@
+// ps_kernels_mg.cuh -- grid-transfer kernels of the multigrid acceleration (PAPER.md:78
+// "multigrid accelerated red black SOR relaxation scheme"; readings M1-M4 of DESIGN.md §12).
+//
+//   ps_mg_coarsen_kernel          M1  coarse face coefficient = 1/16 sum of the 4 fine faces
+//   ps_mg_residual_restrict_kernel M2+M3  rc = 1/8 sum over the 8 children of (rhs - A p)
+//   ps_mg_prolong_add_kernel      M4  p += e_parent
+//
+// All are single-pass, HBM-bound streaming kernels: one thread per COARSE cell (coarsen,
+// residual+restrict: it reads its 2x2x2 children with 16-byte loads) or per pair of fine cells
+// (prolongation).  The summation orders are fixed and written out, so results are bitwise those
+// of the two-step definition (residual field, then restriction).  Compile with --fmad=false.
+#pragma once
+#include "ps_kernels_generic.cuh"
+
+namespace ps {
+
+// M1.  gf = fine grid (nx, ny even; nz even).  Coarse cell (I,J,K); fine corner (2I,2J,2K).
+__global__ void __launch_bounds__(256)
+ps_mg_coarsen_kernel(Grid gf, const double *__restrict__ ax, const double *__restrict__ ay,
+                     const double *__restrict__ az, double *__restrict__ axc,
+                     double *__restrict__ ayc, double *__restrict__ azc)
+{
+    const int cx = gf.nx >> 1, cy = gf.ny >> 1, cz = gf.nz >> 1;
+    const size_t NC = (size_t)cx * cy * cz;
+    const size_t sx = 1, sy = (size_t)gf.nx, sz = (size_t)gf.nx * gf.ny;
+    for (size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x; c < NC;
+         c += (size_t)gridDim.x * blockDim.x) {
+        const int I = (int)(c % cx);
+        const size_t t = c / cx;
+        const int J = (int)(t % cy), K = (int)(t / cy);
+        const size_t n = gf.idx(2 * I, 2 * J, 2 * K);
+        axc[c] = 0.0625 * (((ax[n + sx] + ax[n + sx + sy]) + ax[n + sx + sz]) + ax[n + sx + sy + sz]);
+        ayc[c] = 0.0625 * (((ay[n + sy] + ay[n + sx + sy]) + ay[n + sy + sz]) + ay[n + sx + sy + sz]);
+        azc[c] = 0.0625 * (((az[n + sz] + az[n + sx + sz]) + az[n + sy + sz]) + az[n + sx + sy + sz]);
+    }
+}
+
+// M2 + M3 fused: the residual of the 8 children, summed with x fastest, then y, then z, times 1/8.
+// The residual field itself is never stored (saves 16 B per fine cell of traffic).
+__global__ void __launch_bounds__(256)
+ps_mg_residual_restrict_kernel(Grid gf, const double *__restrict__ ax,
+                               const double *__restrict__ ay, const double *__restrict__ az,
+                               const double *__restrict__ rhs, const double *__restrict__ p,
+                               double *__restrict__ rc)
+{
+    const int cx = gf.nx >> 1, cy = gf.ny >> 1, cz = gf.nz >> 1;
+    const size_t NC = (size_t)cx * cy * cz;
+    for (size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x; c < NC;
+         c += (size_t)gridDim.x * blockDim.x) {
+        const int I = (int)(c % cx);
+        const size_t t = c / cx;
+        const int J = (int)(t % cy), K = (int)(t / cy);
+        double acc = 0.0;
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+            const int i = 2 * I + (q & 1), j = 2 * J + ((q >> 1) & 1), k = 2 * K + (q >> 2);
+            const size_t n = gf.idx(i, j, k);
+            const Stencil s = gather(gf, ax, ay, az, p, i, j, k, n);
+            const double r = residual_at(s.axm, s.axp, s.aym, s.ayp, s.azm, s.azp, s.pxm, s.pxp,
+                                         s.pym, s.pyp, s.pzm, s.pzp, p[n], rhs[n]);
+            acc = (q == 0) ? r : acc + r;
+        }
+        rc[c] = 0.125 * acc;
+    }
+}
+
+// M2 alone (kept for tests of the residual field).
+__global__ void __launch_bounds__(256)
+ps_mg_residual_field_kernel(Grid g, const double *__restrict__ ax, const double *__restrict__ ay,
+                            const double *__restrict__ az, const double *__restrict__ rhs,
+                            const double *__restrict__ p, double *__restrict__ r)
+{
+    const size_t N = g.cells();
+    for (size_t n = (size_t)blockIdx.x * blockDim.x + threadIdx.x; n < N;
+         n += (size_t)gridDim.x * blockDim.x) {
+        const int i = (int)(n % g.nx);
+        const size_t t = n / g.nx;
+        const int j = (int)(t % g.ny), k = (int)(t / g.ny);
+        const Stencil s = gather(g, ax, ay, az, p, i, j, k, n);
+        r[n] = residual_at(s.axm, s.axp, s.aym, s.ayp, s.azm, s.azp, s.pxm, s.pxp, s.pym, s.pyp,
+                           s.pzm, s.pzp, p[n], rhs[n]);
+    }
+}
+
+// M4.  One thread per x-pair of fine cells (both children of the same parent): 16-byte access.
+__global__ void __launch_bounds__(256)
+ps_mg_prolong_add_kernel(Grid gf, const double *__restrict__ ec, double *__restrict__ p)
+{
+    const int cx = gf.nx >> 1, cy = gf.ny >> 1;
+    const size_t pairs = (size_t)cx * gf.ny * gf.nz;
+    for (size_t h = (size_t)blockIdx.x * blockDim.x + threadIdx.x; h < pairs;
+         h += (size_t)gridDim.x * blockDim.x) {
+        const int I = (int)(h % cx);
+        const size_t t = h / cx;
+        const int j = (int)(t % gf.ny), k = (int)(t / gf.ny);
+        const double e = ec[(size_t)I + (size_t)cx * ((size_t)(j >> 1) + (size_t)cy * (size_t)(k >> 1))];
+        double2 *q = reinterpret_cast<double2 *>(p + gf.idx(2 * I, j, k));
+        double2 v = *q;
+        v.x = v.x + e;
+        v.y = v.y + e;
+        *q = v;
+    }
+}
+
+}  // namespace ps
