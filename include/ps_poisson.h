@@ -155,11 +155,15 @@ int ps_timing(ps_ctx *c, double *sweep_ms, long long *sweep_launches);
  * ny stay even and >= 2 after halving and nz is a multiple of 4; coarse face coefficient =
  * 1/16 of the sum of the 4 fine face coefficients on the coarse face; restriction = mean of the
  * 8 children of r = rhs - A p; piecewise-constant prolongation added to p; red-black SOR
- * (omega_s) as smoother (nu1 before, nu2 after) and as coarsest-level solver (coarse_sweeps);
+ * (omega_s) as smoother (nu1 before, nu2 after; on level l multiplied by nu_growth^l up to
+ * nu_max, because coarse levels are cheap and the bubble modes need them solved accurately)
+ * and as coarsest-level solver (coarse_sweeps);
  * gamma = 1 (V cycle) or 2 (W cycle). */
 typedef struct {
     int levels;          /* requested levels, clipped to [1, what the grid allows]            */
-    int nu1, nu2;        /* pre-/post-smoothing sweeps (>= 0)                                  */
+    int nu1, nu2;        /* pre-/post-smoothing sweeps on the finest level (>= 0)              */
+    int nu_growth;       /* level l smooths min(nu * nu_growth^l, nu_max) times (>= 1)         */
+    int nu_max;          /* cap of the per-level count (>= 1; never lowers nu itself)          */
     int coarse_sweeps;   /* sweeps on the coarsest level (>= 1)                                */
     int gamma;           /* 1 = V, 2 = W                                                       */
     double omega_s;      /* relaxation factor of smoother and coarsest solver, in (0,2)        */

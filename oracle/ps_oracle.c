@@ -276,7 +276,16 @@ typedef struct {
 
 /* M6: one cycle on level l.  Coarsest level: coarse_sweeps SOR sweeps.  Otherwise nu1 sweeps,
  * residual, restriction to the rhs of level l+1, zero initial guess there, gamma recursive
- * cycles (1 = V, 2 = W), prolongation added to p, nu2 sweeps. */
+ * cycles (1 = V, 2 = W), prolongation added to p, nu2 sweeps.  On level l the smoothing counts are
+ * min(nu * nu_growth^l, nu_max) (never below nu): coarse levels are cheap and the bubble modes
+ * need them solved accurately (DESIGN.md §12 M6). */
+static int mg_nu(int nu, int l, const ora_mg_params *prm)
+{
+    long long v = nu;
+    for (int q = 0; q < l && v < prm->nu_max; ++q) v *= prm->nu_growth;
+    return (int)(v < prm->nu_max ? v : (nu < prm->nu_max ? prm->nu_max : nu));
+}
+
 static void mg_cycle(mg_level *lv, int l, int nlev, const ora_mg_params *prm)
 {
     mg_level *f = &lv[l];
@@ -286,14 +295,14 @@ static void mg_cycle(mg_level *lv, int l, int nlev, const ora_mg_params *prm)
         return;
     }
     mg_level *c = &lv[l + 1];
-    for (int s = 0; s < prm->nu1; ++s)
+    for (int s = 0, n1 = mg_nu(prm->nu1, l, prm); s < n1; ++s)
         ora_sweep(f->nx, f->ny, f->nz, f->ax, f->ay, f->az, f->rhs, f->p, prm->omega_s);
     ora_mg_residual_field(f->nx, f->ny, f->nz, f->ax, f->ay, f->az, f->rhs, f->p, f->r);
     ora_mg_restrict(f->nx, f->ny, f->nz, f->r, c->rhs);
     memset(c->p, 0, sizeof(double) * (size_t)c->nx * c->ny * c->nz);
     for (int g = 0; g < prm->gamma; ++g) mg_cycle(lv, l + 1, nlev, prm);
     ora_mg_prolong_add(f->nx, f->ny, f->nz, c->p, f->p);
-    for (int s = 0; s < prm->nu2; ++s)
+    for (int s = 0, n2 = mg_nu(prm->nu2, l, prm); s < n2; ++s)
         ora_sweep(f->nx, f->ny, f->nz, f->ax, f->ay, f->az, f->rhs, f->p, prm->omega_s);
 }
 

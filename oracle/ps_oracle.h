@@ -34,7 +34,9 @@ void ora_solve(int nx, int ny, int nz, const double *ax, const double *ay, const
 /* Multigrid acceleration (readings M1-M6 of DESIGN.md §12). */
 typedef struct {
     int levels;          /* requested number of levels (clipped to what the grid allows) */
-    int nu1, nu2;        /* pre- and post-smoothing sweeps */
+    int nu1, nu2;        /* pre- and post-smoothing sweeps on level 0 */
+    int nu_growth;       /* level l smooths min(nu * nu_growth^l, nu_max) times (1 = same everywhere) */
+    int nu_max;          /* cap of the per-level smoothing count */
     int coarse_sweeps;   /* SOR sweeps on the coarsest level */
     int gamma;           /* recursive cycles per level: 1 = V, 2 = W */
     double omega_s;      /* relaxation factor of the smoother and coarsest solver */

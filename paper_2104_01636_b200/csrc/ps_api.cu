@@ -531,20 +531,27 @@ int mg_launch_prolong_add(ps_ctx *f, const double *ec, double *p)
     return PS_OK;
 }
 
-// M6: one cycle on the level of context f.
-int mg_cycle(ps_ctx *f, const ps_mg_params &m, const double *rhs, double *p)
+int mg_nu(int nu, int level, const ps_mg_params &m)
+{
+    long long v = nu;
+    for (int q = 0; q < level && v < m.nu_max; ++q) v *= m.nu_growth;
+    return (int)(v < m.nu_max ? v : (nu < m.nu_max ? m.nu_max : nu));
+}
+
+// M6: one cycle on the level of context f (level index = depth below the finest).
+int mg_cycle(ps_ctx *f, const ps_mg_params &m, const double *rhs, double *p, int level = 0)
 {
     int rc;
     if (!f->child || f->mg_nlev <= 1)
         return run_sweeps(f, rhs, p, m.omega_s, m.coarse_sweeps);
     ps_ctx *k = f->child;
-    if ((rc = run_sweeps(f, rhs, p, m.omega_s, m.nu1))) return rc;
+    if ((rc = run_sweeps(f, rhs, p, m.omega_s, mg_nu(m.nu1, level, m)))) return rc;
     if ((rc = mg_launch_residual_restrict(f, rhs, p, k->lv_rhs))) return rc;
     PS_CUDA(cudaMemsetAsync(k->lv_p, 0, k->g.cells() * sizeof(double), f->stream));
     for (int g = 0; g < m.gamma; ++g)
-        if ((rc = mg_cycle(k, m, k->lv_rhs, k->lv_p))) return rc;
+        if ((rc = mg_cycle(k, m, k->lv_rhs, k->lv_p, level + 1))) return rc;
     if ((rc = mg_launch_prolong_add(f, k->lv_p, p))) return rc;
-    return run_sweeps(f, rhs, p, m.omega_s, m.nu2);
+    return run_sweeps(f, rhs, p, m.omega_s, mg_nu(m.nu2, level, m));
 }
 
 }  // namespace
@@ -554,7 +561,8 @@ extern "C" {
 int ps_mg_setup(ps_ctx *c, const ps_mg_params *prm)
 {
     if (!c || !prm) return PS_EINVAL;
-    if (prm->nu1 < 0 || prm->nu2 < 0 || prm->coarse_sweeps < 1 || prm->gamma < 1 ||
+    if (prm->nu1 < 0 || prm->nu2 < 0 || prm->nu_growth < 1 || prm->nu_max < 1 ||
+        prm->coarse_sweeps < 1 || prm->gamma < 1 ||
         prm->gamma > 2 || !(prm->omega_s > 0.0 && prm->omega_s < 2.0))
         return PS_EINVAL;
     if (!c->have_coef) return PS_ESTATE;

@@ -164,3 +164,37 @@ def test_mg_needs_far_fewer_passes_than_sor_on_a_bubbly_duct(ora):
                         gamma=1, omega_s=1.2)
     assert info.converged and info.sweeps <= 60       # plain SOR: thousands of sweeps (config 1)
     assert abs(ora.residual(coef, w.rhs, p)[1] - info.res_rel) <= 1e-12 * info.res_rel
+
+
+def test_level_dependent_smoothing_counts(ora):
+    """nu_growth = 1 is the plain cycle; with growth the coarse levels get min(nu g^l, nu_max)
+    sweeps: two levels with nu_growth = 3 equal two levels whose coarsest solver runs the same
+    number of sweeps -- checked through a case where level 1 IS the coarsest (growth must not
+    touch coarse_sweeps) and through a 3-level case against hand-unrolled oracle steps."""
+    nx, ny, nz = 8, 8, 16
+    coef = var_coef(ora, nx, ny, nz, 41)
+    rhs = wl.remove_mean(rnd((nz, ny, nx), 42))
+    a, b = np.zeros_like(rhs), np.zeros_like(rhs)
+    ora.mg_solve(coef, rhs, a, 2, 0.0, levels=2, nu1=1, nu2=1, coarse_sweeps=9, omega_s=1.3,
+                 nu_growth=3, nu_max=100)
+    ora.mg_solve(coef, rhs, b, 2, 0.0, levels=2, nu1=1, nu2=1, coarse_sweeps=9, omega_s=1.3)
+    assert np.array_equal(a, b)
+    # 3 levels, nu = 1, growth 3, cap 2: level 0 smooths 1, level 1 smooths min(3, 2) = 2
+    p = np.zeros_like(rhs)
+    ora.mg_solve(coef, rhs, p, 1, 0.0, levels=3, nu1=1, nu2=1, coarse_sweeps=5, omega_s=1.3,
+                 nu_growth=3, nu_max=2)
+    c1 = ora.mg_coarsen(coef)
+    c2 = ora.mg_coarsen(c1)
+    q = np.zeros_like(rhs)
+    ora.sweep(coef, rhs, q, 1.3, 1)
+    r1 = ora.mg_restrict(ora.mg_residual_field(coef, rhs, q))
+    e1 = np.zeros_like(r1)
+    ora.sweep(c1, r1, e1, 1.3, 2)
+    r2 = ora.mg_restrict(ora.mg_residual_field(c1, r1, e1))
+    e2 = np.zeros_like(r2)
+    ora.sweep(c2, r2, e2, 1.3, 5)
+    ora.mg_prolong_add(e2, e1)
+    ora.sweep(c1, r1, e1, 1.3, 2)
+    ora.mg_prolong_add(e1, q)
+    ora.sweep(coef, rhs, q, 1.3, 1)
+    assert np.array_equal(p, q)

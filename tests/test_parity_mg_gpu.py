@@ -67,7 +67,7 @@ def test_transfer_operators_bitwise(torch_cuda, B, ora, shape):
     ora.sweep(coef, w.rhs, p, 1.3, 3)                      # a non-trivial iterate
     with B.PoissonSolver(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz) as s:
         s.set_fraction(dev(torch_cuda, w.F), w.rho_l, w.rho_g)
-        nlev = s.mg_setup(levels=3)
+        nlev = s.mg_setup(levels=3, nu_growth=1)
         assert nlev == min(3, ora.mg_max_levels(w.nx, w.ny, w.nz))
         c = coef
         for level in range(1, nlev):                       # M1, level by level
@@ -85,10 +85,11 @@ def test_transfer_operators_bitwise(torch_cuda, B, ora, shape):
 
 
 PARAMS = [
-    dict(levels=99, nu1=2, nu2=2, coarse_sweeps=20, gamma=1, omega_s=1.2),
-    dict(levels=2, nu1=1, nu2=3, coarse_sweeps=7, gamma=2, omega_s=1.0),     # odd sweep counts
-    dict(levels=3, nu1=2, nu2=2, coarse_sweeps=30, gamma=2, omega_s=1.3),
-    dict(levels=1, nu1=0, nu2=0, coarse_sweeps=5, gamma=1, omega_s=1.5),     # plain SOR
+    dict(levels=99, nu1=2, nu2=2, coarse_sweeps=20, gamma=1, omega_s=1.2, nu_growth=1, nu_max=64),
+    dict(levels=2, nu1=1, nu2=3, coarse_sweeps=7, gamma=2, omega_s=1.0, nu_growth=1, nu_max=64),     # odd sweep counts
+    dict(levels=3, nu1=2, nu2=2, coarse_sweeps=30, gamma=2, omega_s=1.3, nu_growth=1, nu_max=64),
+    dict(levels=1, nu1=0, nu2=0, coarse_sweeps=5, gamma=1, omega_s=1.5, nu_growth=1, nu_max=64),     # plain SOR
+    dict(levels=99, nu1=2, nu2=1, coarse_sweeps=40, gamma=1, omega_s=1.6, nu_growth=4, nu_max=16),
 ]
 
 
@@ -112,7 +113,7 @@ def test_cycles_bitwise(torch_cuda, B, ora, shape, prm):
 
 def test_config1_to_tolerance_same_cycle_count(torch_cuda, B, ora):
     w = wl.make_config(1)
-    prm = dict(levels=3, nu1=2, nu2=2, coarse_sweeps=100, gamma=1, omega_s=1.2)
+    prm = dict(levels=3, nu1=2, nu2=2, coarse_sweeps=100, gamma=1, omega_s=1.2, nu_growth=1, nu_max=64)
     coef = ora.coefficients(w.F, w.rho_l, w.rho_g, w.dx, w.dy, w.dz)
     p_o = np.zeros_like(w.rhs)
     io = ora.mg_solve(coef, w.rhs, p_o, 200, 1e-8, **prm)
@@ -131,7 +132,7 @@ def test_config1_to_tolerance_same_cycle_count(torch_cuda, B, ora):
 
 def test_config3_three_cycles_and_state_errors(torch_cuda, B, ora):
     w = wl.make_config(3)
-    prm = dict(levels=4, nu1=2, nu2=2, coarse_sweeps=40, gamma=1, omega_s=1.2)
+    prm = dict(levels=4, nu1=2, nu2=2, coarse_sweeps=40, gamma=1, omega_s=1.2, nu_growth=1, nu_max=64)
     coef = ora.coefficients(w.F, w.rho_l, w.rho_g, w.dx, w.dy, w.dz)
     p_o = np.zeros_like(w.rhs)
     io = ora.mg_solve(coef, w.rhs, p_o, 3, 0.0, **prm)
