@@ -14,6 +14,7 @@
 #include "ps_kernels_generic.cuh"
 #include "ps_kernels_zmarch.cuh"
 #include "ps_kernels_mg.cuh"
+#include "ps_kernels_resident.cuh"
 
 namespace {
 
@@ -31,6 +32,8 @@ int cuda_fail(cudaError_t e)
         if (e_ != cudaSuccess) return cuda_fail(e_);    \
     } while (0)
 
+constexpr size_t ps_resident_max_cells = 131072;
+
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 }  // namespace
@@ -44,6 +47,7 @@ struct ps_ctx {
     int variant;           // resolved
     bool have_coef;
     int sm_count;
+    int coop;              // device supports cooperative launches
     long long launches;
     // workspace
     void *ws;
@@ -110,10 +114,15 @@ int ensure_workspace(ps_ctx *c)
 int resolve_variant(const ps_ctx *c, int req)
 {
     const bool fused_ok = c->fused.ok;
+    // small grids live in L2 and are bound by launch / pipeline start-up latency: many sweeps per
+    // cooperative launch win there (measured cross-over between 65 k and 524 k cells)
+    if (req == PS_KERNEL_AUTO && c->coop && c->g.cells() <= (size_t)ps_resident_max_cells)
+        return PS_KERNEL_RESIDENT;
     if (req == PS_KERNEL_AUTO) return fused_ok ? PS_KERNEL_FUSED : PS_KERNEL_TWOPASS;
     if (req == PS_KERNEL_FUSED && !fused_ok) return -1;
     if (req == PS_KERNEL_FUSED_T2) return -1;          // not built yet
-    if (req < PS_KERNEL_AUTO || req > PS_KERNEL_FUSED_T2) return -1;
+    if (req == PS_KERNEL_RESIDENT && !c->coop) return -1;
+    if (req < PS_KERNEL_AUTO || req > PS_KERNEL_RESIDENT) return -1;
     return req;
 }
 
@@ -172,6 +181,24 @@ int run_sweeps_untimed(ps_ctx *c, const double *rhs, double *p, double omega, in
         }
         return PS_OK;
     }
+    if (c->variant == PS_KERNEL_RESIDENT) {
+        const size_t items = (size_t)((c->g.nx + 1) / 2) * c->g.ny * c->g.nz;
+        int threads = ps::RES_THREADS;
+        size_t blocks = (items + threads - 1) / threads;
+        if (items <= (size_t)ps::RES_THREADS_ONE) { threads = ps::RES_THREADS_ONE; blocks = 1; }
+        if (blocks > (size_t)c->sm_count) blocks = (size_t)c->sm_count;
+        if ((long long)n * 2 * (long long)blocks > 0x7fffffffLL) return PS_EINVAL;
+        ps::Grid g = c->g;
+        const double *ax = c->ax, *ay = c->ay, *az = c->az;
+        unsigned *ctr = (unsigned *)c->done;
+        if (blocks > 1) PS_CUDA(cudaMemsetAsync(ctr, 0, sizeof(unsigned), c->stream));
+        void *args[] = {&g, &ax, &ay, &az, &rhs, &p, &omega, &n, &ctr};
+        PS_CUDA(cudaLaunchCooperativeKernel((const void *)ps::ps_resident_sweeps_kernel,
+                                            dim3((unsigned)blocks), dim3((unsigned)threads), args,
+                                            0, c->stream));
+        c->launches++;
+        return PS_OK;
+    }
     double *src = p, *dst = c->p_alt;
     int left = n;
     while (left > 0) {
@@ -221,6 +248,8 @@ int ps_create(ps_ctx **out, int nx, int ny, int nz, double dx, double dy, double
     int dev = 0, sms = 0;
     PS_CUDA(cudaGetDevice(&dev));
     PS_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    int coop = 0;
+    PS_CUDA(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
     ps_ctx *c = new (std::nothrow) ps_ctx();
     if (!c) return PS_ENOMEM;
     c->g = ps::Grid{nx, ny, nz};
@@ -229,6 +258,7 @@ int ps_create(ps_ctx **out, int nx, int ny, int nz, double dx, double dy, double
     c->dx = dx; c->dy = dy; c->dz = dz;
     c->K = 50;
     c->sm_count = sms;
+    c->coop = coop;
     c->nparts = (int)((c->g.cells() + ps::RED_CHUNK - 1) / ps::RED_CHUNK);
     cudaError_t e = cudaMallocHost((void **)&c->h_scal, 4 * sizeof(double));
     if (e != cudaSuccess) { delete c->ev; delete c; return cuda_fail(e); }

@@ -47,12 +47,12 @@ def variants_for(B, w, tunings=((1, 0), (2, 0), (1, 1), (2, 3))):
     (kernel, rows_per_thread, z_chunks); the fused kernel is run in several launch geometries."""
     out = []
     with B.PoissonSolver(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, workspace=False) as s:
-        for v in (B.KERNEL_TWOPASS, B.KERNEL_FUSED, B.KERNEL_FUSED_T2):
+        for v in (B.KERNEL_TWOPASS, B.KERNEL_RESIDENT, B.KERNEL_FUSED, B.KERNEL_FUSED_T2):
             try:
                 s.set_kernel(v)
             except B.PsError:
                 continue
-            if v == B.KERNEL_TWOPASS:
+            if v in (B.KERNEL_TWOPASS, B.KERNEL_RESIDENT):
                 out.append((v, 0, 0))
                 continue
             for rpt, chunks in tunings:
@@ -69,7 +69,7 @@ def make_solver(B, w, variant=None):
     if variant is not None:
         kernel, rpt, chunks = variant
         s.set_kernel(kernel)
-        if kernel != B.KERNEL_TWOPASS:
+        if kernel not in (B.KERNEL_TWOPASS, B.KERNEL_RESIDENT):
             s.set_tuning(rpt, chunks)
     return s
 
