@@ -227,3 +227,46 @@ def mg_solve(coef, rhs: np.ndarray, p: np.ndarray, max_cycles: int, tol: float, 
     if rc != 0:
         raise MemoryError("ora_mg_solve")
     return Info(info.sweeps, bool(info.converged), info.res_abs, info.res_rel, info.rhs_norm)
+
+
+# ----------------------------------------------------------------------------- steps 10-12 (P1-P3)
+def _proj_lib():
+    lib = _load()
+    if not getattr(lib, "_proj_ready", False):
+        dp, i, d = ctypes.POINTER(ctypes.c_double), ctypes.c_int, ctypes.c_double
+        lib.ora_rhs_from_velocity.argtypes = [i, i, i, d, d, d, dp, dp, dp, d, dp]
+        lib.ora_correct_velocity.argtypes = [i, i, i, d, d, d, dp, dp, dp, dp, d, dp, dp, dp]
+        lib.ora_face_divergence.argtypes = [i, i, i, d, d, d, dp, dp, dp, dp, dp, dp, dp, d, dp]
+        for f in ("ora_rhs_from_velocity", "ora_correct_velocity", "ora_face_divergence"):
+            getattr(lib, f).restype = None
+        lib._proj_ready = True
+    return lib
+
+
+def rhs_from_velocity(u, h, dt: float) -> np.ndarray:
+    """P1: rhs = div(u_f)/dt from the cell-centred (ux, uy, uz); h = (dx, dy, dz)."""
+    ux, uy, uz = u
+    nx, ny, nz = _shape(ux)
+    rhs = np.empty_like(ux)
+    _proj_lib().ora_rhs_from_velocity(nx, ny, nz, *h, _p(ux), _p(uy), _p(uz), dt, _p(rhs))
+    return rhs
+
+
+def correct_velocity(coef, p: np.ndarray, u, h, dt: float) -> None:
+    """P2 in place on (ux, uy, uz)."""
+    ax, ay, az = coef
+    ux, uy, uz = u
+    nx, ny, nz = _shape(p)
+    _proj_lib().ora_correct_velocity(nx, ny, nz, *h, _p(ax), _p(ay), _p(az), _p(p), dt,
+                                     _p(ux), _p(uy), _p(uz))
+
+
+def face_divergence(coef, u, p: np.ndarray, h, dt: float) -> np.ndarray:
+    """P3: divergence of the corrected face velocity."""
+    ax, ay, az = coef
+    ux, uy, uz = u
+    nx, ny, nz = _shape(p)
+    div = np.empty_like(p)
+    _proj_lib().ora_face_divergence(nx, ny, nz, *h, _p(ax), _p(ay), _p(az), _p(ux), _p(uy), _p(uz),
+                                    _p(p), dt, _p(div))
+    return div

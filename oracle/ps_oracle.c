@@ -365,3 +365,95 @@ int ora_mg_solve(int nx, int ny, int nz, const double *ax, const double *ay, con
     info->rhs_norm = bn;
     return 0;
 }
+
+/* =====================================================================================
+ * The steps either side of the solve: steps 10-12 of the paper's time
+ * step.  Cell-centred intermediate velocity u^ = (ux, uy, uz); "c->f" is the
+ * linear averaging of PAPER.md:117; walls in x, y carry no normal velocity (no-penetration,
+ * PAPER.md:195), z is periodic.  Readings P1-P3 in DESIGN.md §13.
+ * ===================================================================================== */
+
+/* Face-normal velocities of cell (i,j,k): u^_f = u^_{c->f} (step 10), 0 on walls. */
+static inline void face_velocities(int nx, int ny, int nz, const double *ux, const double *uy,
+                                   const double *uz, int i, int j, int k, double f[6])
+{
+    const int km = (k - 1 + nz) % nz, kp = (k + 1) % nz;
+    const size_t n = IDX(i, j, k);
+    f[0] = (i > 0) ? 0.5 * (ux[IDX(i - 1, j, k)] + ux[n]) : 0.0;          /* x- */
+    f[1] = (i < nx - 1) ? 0.5 * (ux[n] + ux[IDX(i + 1, j, k)]) : 0.0;     /* x+ */
+    f[2] = (j > 0) ? 0.5 * (uy[IDX(i, j - 1, k)] + uy[n]) : 0.0;
+    f[3] = (j < ny - 1) ? 0.5 * (uy[n] + uy[IDX(i, j + 1, k)]) : 0.0;
+    f[4] = 0.5 * (uz[IDX(i, j, km)] + uz[n]);
+    f[5] = 0.5 * (uz[n] + uz[IDX(i, j, kp)]);
+}
+
+/* Face values of (grad p / rho) . n of cell (i,j,k): a_f h (p_nb - p_c) with a_f = (1/h^2)/rho_f
+ * the stored coefficient (0 on walls, where p is read at the clamped index). */
+static inline void face_gradients(int nx, int ny, int nz, double dx, double dy, double dz,
+                                  const double *ax, const double *ay, const double *az,
+                                  const double *p, int i, int j, int k, double g[6])
+{
+    const int km = (k - 1 + nz) % nz, kp = (k + 1) % nz;
+    const size_t n = IDX(i, j, k);
+    const double pc = p[n];
+    const double axm = (i > 0) ? ax[IDX(i - 1, j, k)] : 0.0;
+    const double aym = (j > 0) ? ay[IDX(i, j - 1, k)] : 0.0;
+    g[0] = (axm * dx) * (pc - p[IDX(i > 0 ? i - 1 : 0, j, k)]);
+    g[1] = (ax[n] * dx) * (p[IDX(i < nx - 1 ? i + 1 : nx - 1, j, k)] - pc);
+    g[2] = (aym * dy) * (pc - p[IDX(i, j > 0 ? j - 1 : 0, k)]);
+    g[3] = (ay[n] * dy) * (p[IDX(i, j < ny - 1 ? j + 1 : ny - 1, k)] - pc);
+    g[4] = (az[IDX(i, j, km)] * dz) * (pc - p[IDX(i, j, km)]);
+    g[5] = (az[n] * dz) * (p[IDX(i, j, kp)] - pc);
+}
+
+/* P1 (step 11, right-hand side): rhs = div(u^_f) / dt. */
+void ora_rhs_from_velocity(int nx, int ny, int nz, double dx, double dy, double dz,
+                           const double *ux, const double *uy, const double *uz, double dt,
+                           double *rhs)
+{
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) {
+                double f[6];
+                face_velocities(nx, ny, nz, ux, uy, uz, i, j, k, f);
+                const double div = (((f[1] - f[0]) / dx) + ((f[3] - f[2]) / dy))
+                                   + ((f[5] - f[4]) / dz);
+                rhs[IDX(i, j, k)] = div / dt;
+            }
+}
+
+/* P2 (step 12): u_c <- u^_c - dt (grad p / rho)_{f->c}, f->c the mean of the
+ * two faces of the cell in each direction. */
+void ora_correct_velocity(int nx, int ny, int nz, double dx, double dy, double dz,
+                          const double *ax, const double *ay, const double *az, const double *p,
+                          double dt, double *ux, double *uy, double *uz)
+{
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) {
+                double g[6];
+                face_gradients(nx, ny, nz, dx, dy, dz, ax, ay, az, p, i, j, k, g);
+                const size_t n = IDX(i, j, k);
+                ux[n] = ux[n] - dt * (0.5 * (g[0] + g[1]));
+                uy[n] = uy[n] - dt * (0.5 * (g[2] + g[3]));
+                uz[n] = uz[n] - dt * (0.5 * (g[4] + g[5]));
+            }
+}
+
+/* P3: divergence of the corrected FACE velocity u_f = u^_f - dt (grad p / rho)_f, the quantity
+ * the projection drives to zero: equals dt (rhs - A p) up to rounding. */
+void ora_face_divergence(int nx, int ny, int nz, double dx, double dy, double dz, const double *ax,
+                         const double *ay, const double *az, const double *ux, const double *uy,
+                         const double *uz, const double *p, double dt, double *div)
+{
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) {
+                double f[6], g[6], u[6];
+                face_velocities(nx, ny, nz, ux, uy, uz, i, j, k, f);
+                face_gradients(nx, ny, nz, dx, dy, dz, ax, ay, az, p, i, j, k, g);
+                for (int q = 0; q < 6; ++q) u[q] = f[q] - dt * g[q];
+                div[IDX(i, j, k)] = (((u[1] - u[0]) / dx) + ((u[3] - u[2]) / dy))
+                                    + ((u[5] - u[4]) / dz);
+            }
+}

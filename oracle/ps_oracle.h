@@ -53,6 +53,17 @@ int ora_mg_solve(int nx, int ny, int nz, const double *ax, const double *ay, con
                  const double *rhs, double *p, const ora_mg_params *prm, int max_cycles,
                  double tol, ora_info *info);
 
+/* Steps 10-12 of the paper's time step around the solve. */
+void ora_rhs_from_velocity(int nx, int ny, int nz, double dx, double dy, double dz,
+                           const double *ux, const double *uy, const double *uz, double dt,
+                           double *rhs);
+void ora_correct_velocity(int nx, int ny, int nz, double dx, double dy, double dz,
+                          const double *ax, const double *ay, const double *az, const double *p,
+                          double dt, double *ux, double *uy, double *uz);
+void ora_face_divergence(int nx, int ny, int nz, double dx, double dy, double dz, const double *ax,
+                         const double *ay, const double *az, const double *ux, const double *uy,
+                         const double *uz, const double *p, double dt, double *div);
+
 #ifdef __cplusplus
 }
 #endif
