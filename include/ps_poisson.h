@@ -191,6 +191,27 @@ int ps_mg_export_coarse(ps_ctx *c, int level, double *ax_dev, double *ay_dev, do
 int ps_mg_residual_restrict(ps_ctx *c, const double *rhs_dev, const double *p_dev, double *rc_dev);
 int ps_mg_prolong_add(ps_ctx *c, const double *ec_dev, double *p_dev);
 
+/* ------------------------------------------------------------------------------------------
+ * The steps either side of the solve (steps 10-12 of the time step; SURVEY.md
+ * §8.f NEXT-2; readings P1-P3 of DESIGN.md §13).  ux, uy, uz: cell-centred intermediate velocity
+ * u^, device arrays in natural layout.  "c->f" is the linear averaging of PAPER.md:117; wall
+ * faces carry no normal velocity, z is periodic.  All three are one asynchronous
+ * launch on the context's stream.  PS_EINVAL: NULL pointer, dt <= 0 or not finite.
+ * PS_ESTATE (correct / face divergence): no coefficients. */
+
+/* rhs = div(u^_f) / dt  (right-hand side of step 11).  Needs no coefficients. */
+int ps_rhs_from_velocity(ps_ctx *c, const double *ux_dev, const double *uy_dev,
+                         const double *uz_dev, double dt, double *rhs_dev);
+
+/* u_c <- u^_c - dt (grad p / rho)_{f->c}  (step 12), in place on ux, uy, uz. */
+int ps_correct_velocity(ps_ctx *c, const double *p_dev, double dt, double *ux_dev, double *uy_dev,
+                        double *uz_dev);
+
+/* div_dev = div(u^_f - dt (grad p / rho)_f): the divergence of the corrected face velocity,
+ * = dt (rhs - A p); what the projection drives to zero. */
+int ps_face_divergence(ps_ctx *c, const double *ux_dev, const double *uy_dev, const double *uz_dev,
+                       const double *p_dev, double dt, double *div_dev);
+
 /* Kernels launched by this context since ps_create (bench.py's gpu_launches). */
 long long ps_launch_count(const ps_ctx *c);
 

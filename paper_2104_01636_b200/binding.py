@@ -27,7 +27,8 @@ SYMBOLS = ("ps_create", "ps_destroy", "ps_workspace_bytes", "ps_set_workspace", 
            "ps_export_coefficients", "ps_solve", "ps_sweeps", "ps_half_sweep", "ps_residual",
            "ps_solve_host", "ps_enable_timing", "ps_timing", "ps_launch_count", "ps_strerror",
            "ps_mg_setup", "ps_mg_levels", "ps_mg_solve", "ps_mg_export_coarse",
-           "ps_mg_residual_restrict", "ps_mg_prolong_add")
+           "ps_mg_residual_restrict", "ps_mg_prolong_add", "ps_rhs_from_velocity",
+           "ps_correct_velocity", "ps_face_divergence")
 
 
 class PsError(RuntimeError):
@@ -101,6 +102,9 @@ def load(path: str | None = None) -> ctypes.CDLL:
     lib.ps_mg_export_coarse.argtypes = [vp, i, vp, vp, vp]
     lib.ps_mg_residual_restrict.argtypes = [vp, vp, vp, vp]
     lib.ps_mg_prolong_add.argtypes = [vp, vp, vp]
+    lib.ps_rhs_from_velocity.argtypes = [vp, vp, vp, vp, d, vp]
+    lib.ps_correct_velocity.argtypes = [vp, vp, d, vp, vp, vp]
+    lib.ps_face_divergence.argtypes = [vp, vp, vp, vp, vp, d, vp]
     lib.ps_strerror.argtypes = [i]
     lib.ps_strerror.restype = ctypes.c_char_p
     if path == _build.LIB:
@@ -300,6 +304,33 @@ class PoissonSolver:
         self._sync_stream()
         _check(self._lib, self._lib.ps_mg_prolong_add(
             self._h, _dev_ptr(ec, self._coarse_shape(1), "ec"), _dev_ptr(p, self.shape, "p")))
+
+    # -- steps 10-12 of the time step around the solve
+    def rhs_from_velocity(self, ux, uy, uz, dt: float, rhs=None):
+        import torch
+        self._sync_stream()
+        if rhs is None:
+            rhs = torch.empty(self.shape, dtype=torch.float64, device="cuda")
+        _check(self._lib, self._lib.ps_rhs_from_velocity(
+            self._h, _dev_ptr(ux, self.shape, "ux"), _dev_ptr(uy, self.shape, "uy"),
+            _dev_ptr(uz, self.shape, "uz"), dt, _dev_ptr(rhs, self.shape, "rhs")))
+        return rhs
+
+    def correct_velocity(self, p, dt: float, ux, uy, uz):
+        self._sync_stream()
+        _check(self._lib, self._lib.ps_correct_velocity(
+            self._h, _dev_ptr(p, self.shape, "p"), dt, _dev_ptr(ux, self.shape, "ux"),
+            _dev_ptr(uy, self.shape, "uy"), _dev_ptr(uz, self.shape, "uz")))
+
+    def face_divergence(self, ux, uy, uz, p, dt: float):
+        import torch
+        self._sync_stream()
+        div = torch.empty(self.shape, dtype=torch.float64, device="cuda")
+        _check(self._lib, self._lib.ps_face_divergence(
+            self._h, _dev_ptr(ux, self.shape, "ux"), _dev_ptr(uy, self.shape, "uy"),
+            _dev_ptr(uz, self.shape, "uz"), _dev_ptr(p, self.shape, "p"), dt,
+            _dev_ptr(div, self.shape, "div")))
+        return div
 
     def solve_host(self, F, rho_l: float, rho_g: float, rhs, p, omega: float, max_sweeps: int,
                    tol: float) -> Info:

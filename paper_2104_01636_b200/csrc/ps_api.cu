@@ -15,6 +15,7 @@
 #include "ps_kernels_zmarch.cuh"
 #include "ps_kernels_mg.cuh"
 #include "ps_kernels_resident.cuh"
+#include "ps_kernels_projection.cuh"
 
 namespace {
 
@@ -690,6 +691,47 @@ int ps_mg_prolong_add(ps_ctx *c, const double *ec_dev, double *p_dev)
 }  // extern "C"
 
 extern "C" {
+
+int ps_rhs_from_velocity(ps_ctx *c, const double *ux_dev, const double *uy_dev,
+                         const double *uz_dev, double dt, double *rhs_dev)
+{
+    if (!c || !ux_dev || !uy_dev || !uz_dev || !rhs_dev) return PS_EINVAL;
+    if (!(dt > 0.0) || !std::isfinite(dt)) return PS_EINVAL;
+    const ps::Spacing h{c->dx, c->dy, c->dz};
+    ps::ps_rhs_from_velocity_kernel<<<grid_for(c, c->g.cells(), 256), 256, 0, c->stream>>>(
+        c->g, h, ux_dev, uy_dev, uz_dev, dt, rhs_dev);
+    c->launches++;
+    PS_CUDA(cudaGetLastError());
+    return PS_OK;
+}
+
+int ps_correct_velocity(ps_ctx *c, const double *p_dev, double dt, double *ux_dev, double *uy_dev,
+                        double *uz_dev)
+{
+    if (!c || !p_dev || !ux_dev || !uy_dev || !uz_dev) return PS_EINVAL;
+    if (!(dt > 0.0) || !std::isfinite(dt)) return PS_EINVAL;
+    if (!c->have_coef) return PS_ESTATE;
+    const ps::Spacing h{c->dx, c->dy, c->dz};
+    ps::ps_correct_velocity_kernel<<<grid_for(c, c->g.cells(), 256), 256, 0, c->stream>>>(
+        c->g, h, c->ax, c->ay, c->az, p_dev, dt, ux_dev, uy_dev, uz_dev);
+    c->launches++;
+    PS_CUDA(cudaGetLastError());
+    return PS_OK;
+}
+
+int ps_face_divergence(ps_ctx *c, const double *ux_dev, const double *uy_dev, const double *uz_dev,
+                       const double *p_dev, double dt, double *div_dev)
+{
+    if (!c || !ux_dev || !uy_dev || !uz_dev || !p_dev || !div_dev) return PS_EINVAL;
+    if (!(dt > 0.0) || !std::isfinite(dt)) return PS_EINVAL;
+    if (!c->have_coef) return PS_ESTATE;
+    const ps::Spacing h{c->dx, c->dy, c->dz};
+    ps::ps_face_divergence_kernel<<<grid_for(c, c->g.cells(), 256), 256, 0, c->stream>>>(
+        c->g, h, c->ax, c->ay, c->az, ux_dev, uy_dev, uz_dev, p_dev, dt, div_dev);
+    c->launches++;
+    PS_CUDA(cudaGetLastError());
+    return PS_OK;
+}
 
 const char *ps_strerror(int code)
 {
