@@ -59,10 +59,10 @@ ps_coef_build_kernel(Grid g, double cx, double cy, double cz, double rho_l, doub
     const size_t plane = (size_t)g.nx * g.ny;
     for (size_t n = (size_t)blockIdx.x * blockDim.x + threadIdx.x; n < N;
          n += (size_t)gridDim.x * blockDim.x) {
-        const int i = (int)(n % g.nx);
-        const size_t t = n / g.nx;
-        const int j = (int)(t % g.ny);
-        const int k = (int)(t / g.ny);
+        const int i = (int)((unsigned)n % (unsigned)g.nx);
+        const unsigned t = (unsigned)n / (unsigned)g.nx;
+        const int j = (int)(t % (unsigned)g.ny);
+        const int k = (int)(t / (unsigned)g.ny);
         const double Fc = F[n];
         const double rc = (rho_l * Fc) + (rho_g * (1.0 - Fc));
         double vx = 0.0, vy = 0.0;
@@ -127,10 +127,10 @@ ps_half_sweep_kernel(Grid g, const double *__restrict__ ax, const double *__rest
     const size_t total = (size_t)hx * g.ny * g.nz;
     for (size_t h = (size_t)blockIdx.x * blockDim.x + threadIdx.x; h < total;
          h += (size_t)gridDim.x * blockDim.x) {
-        const int ih = (int)(h % hx);
-        const size_t t = h / hx;
-        const int j = (int)(t % g.ny);
-        const int k = (int)(t / g.ny);
+        const int ih = (int)((unsigned)h % (unsigned)hx);
+        const unsigned t = (unsigned)h / (unsigned)hx;
+        const int j = (int)(t % (unsigned)g.ny);
+        const int k = (int)(t / (unsigned)g.ny);
         const int i = 2 * ih + ((j + k + colour) & 1);
         if (i >= g.nx) continue;
         const size_t n = g.idx(i, j, k);
@@ -185,10 +185,10 @@ ps_residual_partial_kernel(Grid g, const double *__restrict__ ax, const double *
     for (int m = 0; m < RED_CHUNK / RED_THREADS; ++m) {
         const size_t n = base + (size_t)m * RED_THREADS + threadIdx.x;
         if (n < N) {
-            const int i = (int)(n % g.nx);
-            const size_t t = n / g.nx;
-            const int j = (int)(t % g.ny);
-            const int k = (int)(t / g.ny);
+            const int i = (int)((unsigned)n % (unsigned)g.nx);
+            const unsigned t = (unsigned)n / (unsigned)g.nx;
+            const int j = (int)(t % (unsigned)g.ny);
+            const int k = (int)(t / (unsigned)g.ny);
             const Stencil s = gather(g, ax, ay, az, p, i, j, k, n);
             const double b = rhs[n];
             const double r = residual_at(s.axm, s.axp, s.aym, s.ayp, s.azm, s.azp, s.pxm, s.pxp,

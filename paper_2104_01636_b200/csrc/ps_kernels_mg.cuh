@@ -25,9 +25,9 @@ ps_mg_coarsen_kernel(Grid gf, const double *__restrict__ ax, const double *__res
     const size_t sx = 1, sy = (size_t)gf.nx, sz = (size_t)gf.nx * gf.ny;
     for (size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x; c < NC;
          c += (size_t)gridDim.x * blockDim.x) {
-        const int I = (int)(c % cx);
-        const size_t t = c / cx;
-        const int J = (int)(t % cy), K = (int)(t / cy);
+        const int I = (int)((unsigned)c % (unsigned)cx);
+        const unsigned t = (unsigned)c / (unsigned)cx;
+        const int J = (int)(t % (unsigned)cy), K = (int)(t / (unsigned)cy);
         const size_t n = gf.idx(2 * I, 2 * J, 2 * K);
         axc[c] = 0.0625 * (((ax[n + sx] + ax[n + sx + sy]) + ax[n + sx + sz]) + ax[n + sx + sy + sz]);
         ayc[c] = 0.0625 * (((ay[n + sy] + ay[n + sx + sy]) + ay[n + sy + sz]) + ay[n + sx + sy + sz]);
@@ -47,9 +47,9 @@ ps_mg_residual_restrict_kernel(Grid gf, const double *__restrict__ ax,
     const size_t NC = (size_t)cx * cy * cz;
     for (size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x; c < NC;
          c += (size_t)gridDim.x * blockDim.x) {
-        const int I = (int)(c % cx);
-        const size_t t = c / cx;
-        const int J = (int)(t % cy), K = (int)(t / cy);
+        const int I = (int)((unsigned)c % (unsigned)cx);
+        const unsigned t = (unsigned)c / (unsigned)cx;
+        const int J = (int)(t % (unsigned)cy), K = (int)(t / (unsigned)cy);
         double acc = 0.0;
 #pragma unroll
         for (int q = 0; q < 8; ++q) {
@@ -73,9 +73,9 @@ ps_mg_residual_field_kernel(Grid g, const double *__restrict__ ax, const double 
     const size_t N = g.cells();
     for (size_t n = (size_t)blockIdx.x * blockDim.x + threadIdx.x; n < N;
          n += (size_t)gridDim.x * blockDim.x) {
-        const int i = (int)(n % g.nx);
-        const size_t t = n / g.nx;
-        const int j = (int)(t % g.ny), k = (int)(t / g.ny);
+        const int i = (int)((unsigned)n % (unsigned)g.nx);
+        const unsigned t = (unsigned)n / (unsigned)g.nx;
+        const int j = (int)(t % (unsigned)g.ny), k = (int)(t / (unsigned)g.ny);
         const Stencil s = gather(g, ax, ay, az, p, i, j, k, n);
         r[n] = residual_at(s.axm, s.axp, s.aym, s.ayp, s.azm, s.azp, s.pxm, s.pxp, s.pym, s.pyp,
                            s.pzm, s.pzp, p[n], rhs[n]);
@@ -90,9 +90,9 @@ ps_mg_prolong_add_kernel(Grid gf, const double *__restrict__ ec, double *__restr
     const size_t pairs = (size_t)cx * gf.ny * gf.nz;
     for (size_t h = (size_t)blockIdx.x * blockDim.x + threadIdx.x; h < pairs;
          h += (size_t)gridDim.x * blockDim.x) {
-        const int I = (int)(h % cx);
-        const size_t t = h / cx;
-        const int j = (int)(t % gf.ny), k = (int)(t / gf.ny);
+        const int I = (int)((unsigned)h % (unsigned)cx);
+        const unsigned t = (unsigned)h / (unsigned)cx;
+        const int j = (int)(t % (unsigned)gf.ny), k = (int)(t / (unsigned)gf.ny);
         const double e = ec[(size_t)I + (size_t)cx * ((size_t)(j >> 1) + (size_t)cy * (size_t)(k >> 1))];
         double2 *q = reinterpret_cast<double2 *>(p + gf.idx(2 * I, j, k));
         double2 v = *q;

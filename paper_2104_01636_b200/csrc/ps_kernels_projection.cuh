@@ -17,10 +17,10 @@ struct Spacing { double dx, dy, dz; };
 
 __device__ __forceinline__ void cell_of(const Grid &g, size_t n, int &i, int &j, int &k)
 {
-    i = (int)(n % g.nx);
-    const size_t t = n / g.nx;
-    j = (int)(t % g.ny);
-    k = (int)(t / g.ny);
+    i = (int)((unsigned)n % (unsigned)g.nx);
+    const unsigned t = (unsigned)n / (unsigned)g.nx;
+    j = (int)(t % (unsigned)g.ny);
+    k = (int)(t / (unsigned)g.ny);
 }
 
 // f[0..5] = x-, x+, y-, y+, z-, z+ face-normal velocities of cell n.

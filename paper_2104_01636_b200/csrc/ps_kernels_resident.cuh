@@ -45,10 +45,10 @@ ps_resident_sweeps_kernel(Grid g, const double *__restrict__ ax, const double *_
     for (int s = 0; s < 2 * nsweeps; ++s) {
         const int colour = s & 1;
         for (size_t h = (size_t)blockIdx.x * blockDim.x + threadIdx.x; h < total; h += stride) {
-            const int ih = (int)(h % hx);
-            const size_t t = h / hx;
-            const int j = (int)(t % g.ny);
-            const int k = (int)(t / g.ny);
+            const int ih = (int)((unsigned)h % (unsigned)hx);
+            const unsigned t = (unsigned)h / (unsigned)hx;
+            const int j = (int)(t % (unsigned)g.ny);
+            const int k = (int)(t / (unsigned)g.ny);
             const int i = 2 * ih + ((j + k + colour) & 1);
             if (i >= g.nx) continue;
             const size_t n = g.idx(i, j, k);
