@@ -212,6 +212,15 @@ int ps_correct_velocity(ps_ctx *c, const double *p_dev, double dt, double *ux_de
 int ps_face_divergence(ps_ctx *c, const double *ux_dev, const double *uy_dev, const double *uz_dev,
                        const double *p_dev, double dt, double *div_dev);
 
+/* Right-hand side of the sharp-surface-force pressure p~ (eqs (6)-(7); SURVEY.md
+ * §8.f NEXT-3; reading T1 of DESIGN.md §14): rhs_c = - sum_f a_f (sigma kappa_f)(F_nb - F_c) with
+ * kappa_f the linear c->f average of the cell curvatures kappa_dev and F_dev the liquid fraction
+ * the coefficients were built from.  The p~ system is then solved with ps_solve / ps_mg_solve on
+ * the same coefficients (a second right-hand side per coefficient set).  One asynchronous launch.
+ * PS_EINVAL: NULL pointer, sigma not finite.  PS_ESTATE: no coefficients. */
+int ps_ssf_rhs(ps_ctx *c, const double *F_dev, const double *kappa_dev, double sigma,
+               double *rhs_dev);
+
 /* Kernels launched by this context since ps_create (bench.py's gpu_launches). */
 long long ps_launch_count(const ps_ctx *c);
 

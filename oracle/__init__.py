@@ -270,3 +270,17 @@ def face_divergence(coef, u, p: np.ndarray, h, dt: float) -> np.ndarray:
     _proj_lib().ora_face_divergence(nx, ny, nz, *h, _p(ax), _p(ay), _p(az), _p(ux), _p(uy), _p(uz),
                                     _p(p), dt, _p(div))
     return div
+
+
+# ----------------------------------------------------------------------------- SSF rhs (T1)
+def ssf_rhs(coef, F: np.ndarray, kappa: np.ndarray, sigma: float) -> np.ndarray:
+    """rhs of the p~ system: -sum_f a_f (sigma kappa_f)(F_nb - F_c)."""
+    ax, ay, az = coef
+    nx, ny, nz = _shape(F)
+    lib = _load()
+    dp, i, d = ctypes.POINTER(ctypes.c_double), ctypes.c_int, ctypes.c_double
+    lib.ora_ssf_rhs.argtypes = [i, i, i, dp, dp, dp, dp, dp, d, dp]
+    lib.ora_ssf_rhs.restype = None
+    rhs = np.empty_like(F)
+    lib.ora_ssf_rhs(nx, ny, nz, _p(ax), _p(ay), _p(az), _p(F), _p(kappa), sigma, _p(rhs))
+    return rhs

@@ -457,3 +457,36 @@ void ora_face_divergence(int nx, int ny, int nz, double dx, double dy, double dz
                                     + ((u[5] - u[4]) / dz);
             }
 }
+
+/* =====================================================================================
+ * Second right-hand side through the same solver: the sharp-surface-force
+ * pressure p~ of PAPER.md:70-78, eqs (6)-(7): sigma kappa n delta = -grad p~ enters
+ * div(grad p~ / rho) = 0 "as a source term".  Reading (T1): n delta = grad alpha
+ * (alpha = liquid fraction F), face curvature kappa_f by the linear c->f average,
+ * so on every face (grad p~ / rho)_f = -sigma kappa_f (grad F / rho)_f and
+ *     sum_f a_f (p~_nb - p~_c) = - sum_f a_f (sigma kappa_f) (F_nb - F_c)  =: rhs_c.
+ * With an exact constant curvature the solution is p~ = sigma kappa (1 - F) + const: the jump
+ * sigma kappa across the interface, and a face force balance that vanishes identically
+ * ("spurious velocities ... reduce to machine zero").
+ * ===================================================================================== */
+void ora_ssf_rhs(int nx, int ny, int nz, const double *ax, const double *ay, const double *az,
+                 const double *F, const double *kappa, double sigma, double *rhs)
+{
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) {
+                const int km = (k - 1 + nz) % nz, kp = (k + 1) % nz;
+                const size_t n = IDX(i, j, k);
+                const size_t nb[6] = {IDX(i > 0 ? i - 1 : 0, j, k), IDX(i < nx - 1 ? i + 1 : nx - 1, j, k),
+                                      IDX(i, j > 0 ? j - 1 : 0, k), IDX(i, j < ny - 1 ? j + 1 : ny - 1, k),
+                                      IDX(i, j, km), IDX(i, j, kp)};
+                const double a[6] = {(i > 0) ? ax[nb[0]] : 0.0, ax[n], (j > 0) ? ay[nb[2]] : 0.0,
+                                     ay[n], az[nb[4]], az[n]};
+                double t[6];
+                for (int q = 0; q < 6; ++q) {
+                    const double kf = 0.5 * (kappa[n] + kappa[nb[q]]);
+                    t[q] = (a[q] * (sigma * kf)) * (F[nb[q]] - F[n]);
+                }
+                rhs[n] = -(((((t[0] + t[1]) + t[2]) + t[3]) + t[4]) + t[5]);
+            }
+}

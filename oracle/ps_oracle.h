@@ -64,6 +64,10 @@ void ora_face_divergence(int nx, int ny, int nz, double dx, double dy, double dz
                          const double *ay, const double *az, const double *ux, const double *uy,
                          const double *uz, const double *p, double dt, double *div);
 
+/* Sharp-surface-force right-hand side for p~ (eqs (6)-(7)). */
+void ora_ssf_rhs(int nx, int ny, int nz, const double *ax, const double *ay, const double *az,
+                 const double *F, const double *kappa, double sigma, double *rhs);
+
 #ifdef __cplusplus
 }
 #endif

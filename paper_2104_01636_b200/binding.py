@@ -28,7 +28,7 @@ SYMBOLS = ("ps_create", "ps_destroy", "ps_workspace_bytes", "ps_set_workspace", 
            "ps_solve_host", "ps_enable_timing", "ps_timing", "ps_launch_count", "ps_strerror",
            "ps_mg_setup", "ps_mg_levels", "ps_mg_solve", "ps_mg_export_coarse",
            "ps_mg_residual_restrict", "ps_mg_prolong_add", "ps_rhs_from_velocity",
-           "ps_correct_velocity", "ps_face_divergence")
+           "ps_correct_velocity", "ps_face_divergence", "ps_ssf_rhs")
 
 
 class PsError(RuntimeError):
@@ -105,6 +105,7 @@ def load(path: str | None = None) -> ctypes.CDLL:
     lib.ps_rhs_from_velocity.argtypes = [vp, vp, vp, vp, d, vp]
     lib.ps_correct_velocity.argtypes = [vp, vp, d, vp, vp, vp]
     lib.ps_face_divergence.argtypes = [vp, vp, vp, vp, vp, d, vp]
+    lib.ps_ssf_rhs.argtypes = [vp, vp, vp, d, vp]
     lib.ps_strerror.argtypes = [i]
     lib.ps_strerror.restype = ctypes.c_char_p
     if path == _build.LIB:
@@ -331,6 +332,16 @@ class PoissonSolver:
             _dev_ptr(uz, self.shape, "uz"), _dev_ptr(p, self.shape, "p"), dt,
             _dev_ptr(div, self.shape, "div")))
         return div
+
+    def ssf_rhs(self, F, kappa, sigma: float):
+        """rhs of the sharp-surface-force pressure system."""
+        import torch
+        self._sync_stream()
+        rhs = torch.empty(self.shape, dtype=torch.float64, device="cuda")
+        _check(self._lib, self._lib.ps_ssf_rhs(
+            self._h, _dev_ptr(F, self.shape, "F"), _dev_ptr(kappa, self.shape, "kappa"), sigma,
+            _dev_ptr(rhs, self.shape, "rhs")))
+        return rhs
 
     def solve_host(self, F, rho_l: float, rho_g: float, rhs, p, omega: float, max_sweeps: int,
                    tol: float) -> Info:

@@ -733,6 +733,18 @@ int ps_face_divergence(ps_ctx *c, const double *ux_dev, const double *uy_dev, co
     return PS_OK;
 }
 
+int ps_ssf_rhs(ps_ctx *c, const double *F_dev, const double *kappa_dev, double sigma,
+               double *rhs_dev)
+{
+    if (!c || !F_dev || !kappa_dev || !rhs_dev || !std::isfinite(sigma)) return PS_EINVAL;
+    if (!c->have_coef) return PS_ESTATE;
+    ps::ps_ssf_rhs_kernel<<<grid_for(c, c->g.cells(), 256), 256, 0, c->stream>>>(
+        c->g, c->ax, c->ay, c->az, F_dev, kappa_dev, sigma, rhs_dev);
+    c->launches++;
+    PS_CUDA(cudaGetLastError());
+    return PS_OK;
+}
+
 const char *ps_strerror(int code)
 {
     switch (code) {

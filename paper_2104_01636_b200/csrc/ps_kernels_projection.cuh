@@ -118,3 +118,39 @@ ps_face_divergence_kernel(Grid g, Spacing h, const double *__restrict__ ax,
 }
 
 }  // namespace ps
+
+// ---------------------------------------------------------------------------------------------
+// Sharp-surface-force right-hand side of the p~ system (eqs (6)-(7)):
+//   rhs_c = - sum_f a_f (sigma kappa_f) (F_nb - F_c),  kappa_f = 0.5 (kappa_c + kappa_nb).
+// One thread per cell; F 8 + kappa 8 + coefficients 24 read, 8 written = 48 B/cell.
+namespace ps {
+
+__global__ void __launch_bounds__(256)
+ps_ssf_rhs_kernel(Grid g, const double *__restrict__ ax, const double *__restrict__ ay,
+                  const double *__restrict__ az, const double *__restrict__ F,
+                  const double *__restrict__ kappa, double sigma, double *__restrict__ rhs)
+{
+    const size_t N = g.cells();
+    for (size_t n = (size_t)blockIdx.x * blockDim.x + threadIdx.x; n < N;
+         n += (size_t)gridDim.x * blockDim.x) {
+        int i, j, k;
+        cell_of(g, n, i, j, k);
+        const size_t plane = (size_t)g.nx * g.ny;
+        const size_t nzm = (k > 0) ? n - plane : n + plane * (size_t)(g.nz - 1);
+        const size_t nzp = (k + 1 < g.nz) ? n + plane : n - plane * (size_t)(g.nz - 1);
+        const size_t nb[6] = {(i > 0) ? n - 1 : n, (i < g.nx - 1) ? n + 1 : n,
+                              (j > 0) ? n - g.nx : n, (j < g.ny - 1) ? n + g.nx : n, nzm, nzp};
+        const double a[6] = {(i > 0) ? ax[n - 1] : 0.0, ax[n], (j > 0) ? ay[n - g.nx] : 0.0, ay[n],
+                             az[nzm], az[n]};
+        const double Fc = F[n], kc = kappa[n];
+        double t[6];
+#pragma unroll
+        for (int q = 0; q < 6; ++q) {
+            const double kf = 0.5 * (kc + kappa[nb[q]]);
+            t[q] = (a[q] * (sigma * kf)) * (F[nb[q]] - Fc);
+        }
+        rhs[n] = -(((((t[0] + t[1]) + t[2]) + t[3]) + t[4]) + t[5]);
+    }
+}
+
+}  // namespace ps

@@ -240,3 +240,25 @@ def random_fraction(nx: int, ny: int, nz: int, seed: int, sub: int = 4) -> np.nd
     idx = np.arange(nx * ny * nz, dtype=np.uint64)
     m = (uniform01(seed, 2, idx) * (sub ** 3 + 1)).astype(np.int64)
     return (m.astype(np.float64) / float(sub ** 3)).reshape(nz, ny, nx)
+
+
+# ----------------------------------------------------------------------------- SSF inputs
+SIGMA = 0.072                   # surface tension of air-water, N/m (PAPER.md:220 fluid pair)
+
+
+def curvature_field(nx: int, ny: int, nz: int, centres: np.ndarray, diameter: int,
+                    h: float) -> np.ndarray:
+    """Exact interface curvature kappa = 2/R of every sphere (R = diameter/2 cells of size h),
+    stored in all cells of the sphere's bounding box grown by one cell (z wrapped); 0 elsewhere.
+    This is the "exact analytical curvature" case of PAPER.md:78; the height-function estimate of
+    step 5 is out of scope.  Input generator only: no solver arithmetic."""
+    kappa = np.zeros((nz, ny, nx), dtype=np.float64)
+    if len(centres):
+        R = diameter // 2
+        val = 2.0 / (R * h)
+        for cx, cy, cz in np.asarray(centres, dtype=np.int64):
+            kz = (np.arange(cz - R - 1, cz + R + 1) % nz)
+            ys = np.arange(max(cy - R - 1, 0), min(cy + R + 1, ny))
+            xs = np.arange(max(cx - R - 1, 0), min(cx + R + 1, nx))
+            kappa[kz[:, None, None], ys[None, :, None], xs[None, None, :]] = val
+    return kappa
