@@ -41,8 +41,7 @@ UNIT = "Gcell-updates/s"
 # algorithmic bytes per cell per sweep-kernel launch:
 #   twopass: one colour per launch, M1 = 40 B/cell/launch (80 B per cell-update)
 #   fused:   one sweep per launch,  M2 = 48 B/cell/launch (48 B per cell-update)
-#   fused_t2: two sweeps per launch, still 48 B/cell/launch (24 B per cell-update)
-ALGO_BYTES_PER_CELL_LAUNCH = {"twopass": 40.0, "fused": 48.0, "fused_t2": 48.0,
+ALGO_BYTES_PER_CELL_LAUNCH = {"twopass": 40.0, "fused": 48.0,
                               "resident": 80.0}   # resident: L2-resident grids only, per sweep
 
 
@@ -55,7 +54,7 @@ def parse_args():
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json config 1..5 (default 4)")
     ap.add_argument("--sweeps", type=int, default=0, help="sweeps per step (default: the config's)")
     ap.add_argument("--kernel", default="auto",
-                    choices=["auto", "twopass", "fused", "fused_t2", "resident"])
+                    choices=["auto", "twopass", "fused", "resident"])
     ap.add_argument("--no-mg", action="store_true", help="skip the multigrid time-to-1e-8 leg")
     ap.add_argument("--rpt", type=int, default=0, help="fused kernel: rows per thread (0 = auto)")
     ap.add_argument("--zchunks", type=int, default=0, help="fused kernel: z chunks (0 = auto)")
@@ -226,7 +225,7 @@ def run_ours(args, rank):
     sweeps = sweeps_for(args.config, args.sweeps)
     shape = (w.nz, w.ny, w.nx)
     kernel = {"auto": binding.KERNEL_AUTO, "twopass": binding.KERNEL_TWOPASS,
-              "fused": binding.KERNEL_FUSED, "fused_t2": binding.KERNEL_FUSED_T2,
+              "fused": binding.KERNEL_FUSED,
               "resident": binding.KERNEL_RESIDENT}[args.kernel]
 
     F_h = torch.from_numpy(w.F).pin_memory()
@@ -332,8 +331,7 @@ def run_ours(args, rank):
                          else "L2-resident working set (not an HBM measurement)",
                    "parallelism": "replicas" if rank.world > 1 else "single GPU"},
         "final_res_rel": info.res_rel,
-        "sweep_only_gcells_per_s": w.cells * (sweep_launches * (0.5 if kname == "twopass" else
-                                              2.0 if kname == "fused_t2" else 1.0))
+        "sweep_only_gcells_per_s": w.cells * (sweep_launches * (0.5 if kname == "twopass" else 1.0))
                                    / (sweep_ms / 1e3) / 1e9 if sweep_ms > 0 else None,
         "gpu_launches": launches,
         "clocks": clk,

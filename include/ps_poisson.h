@@ -47,9 +47,9 @@ extern "C" {
 /* Sweep kernel variants (ps_set_kernel).  All give bitwise identical p. */
 #define PS_KERNEL_AUTO     0   /* fastest variant the grid shape allows                     */
 #define PS_KERNEL_TWOPASS  1   /* generic: one launch per colour, in place, any nx,ny>=1    */
-#define PS_KERNEL_FUSED    2   /* red+black fused in one z-marching pass, ping-pong p       */
-#define PS_KERNEL_FUSED_T2 3   /* two fused sweeps temporally blocked per launch            */
-#define PS_KERNEL_RESIDENT 4   /* L2-resident grids: n sweeps in ONE cooperative launch,    */
+#define PS_KERNEL_FUSED    2   /* red+black fused in one z-marching pass (both half-sweeps  */
+                               /* temporally blocked in one launch), ping-pong p            */
+#define PS_KERNEL_RESIDENT 3   /* L2-resident grids: n sweeps in ONE cooperative launch,    */
                                /* grid-wide barrier per half-sweep, in place, any nx,ny>=1  */
 
 typedef struct ps_ctx ps_ctx;   /* opaque; one per grid */

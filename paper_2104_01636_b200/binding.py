@@ -16,9 +16,9 @@ from dataclasses import dataclass
 from . import build as _build
 
 PS_OK, PS_EINVAL, PS_ESTATE, PS_ECUDA, PS_ENOMEM = 0, -1, -2, -3, -4
-KERNEL_AUTO, KERNEL_TWOPASS, KERNEL_FUSED, KERNEL_FUSED_T2, KERNEL_RESIDENT = 0, 1, 2, 3, 4
+KERNEL_AUTO, KERNEL_TWOPASS, KERNEL_FUSED, KERNEL_RESIDENT = 0, 1, 2, 3
 KERNEL_NAMES = {KERNEL_AUTO: "auto", KERNEL_TWOPASS: "twopass", KERNEL_FUSED: "fused",
-                KERNEL_FUSED_T2: "fused_t2", KERNEL_RESIDENT: "resident"}
+                KERNEL_RESIDENT: "resident"}
 
 # every symbol include/ps_poisson.h declares (tests check the library exports each one)
 SYMBOLS = ("ps_create", "ps_destroy", "ps_workspace_bytes", "ps_set_workspace", "ps_set_stream",

@@ -121,7 +121,6 @@ int resolve_variant(const ps_ctx *c, int req)
         return PS_KERNEL_RESIDENT;
     if (req == PS_KERNEL_AUTO) return fused_ok ? PS_KERNEL_FUSED : PS_KERNEL_TWOPASS;
     if (req == PS_KERNEL_FUSED && !fused_ok) return -1;
-    if (req == PS_KERNEL_FUSED_T2) return -1;          // not built yet
     if (req == PS_KERNEL_RESIDENT && !c->coop) return -1;
     if (req < PS_KERNEL_AUTO || req > PS_KERNEL_RESIDENT) return -1;
     return req;

@@ -47,7 +47,7 @@ def variants_for(B, w, tunings=((1, 0), (2, 0), (1, 1), (2, 3))):
     (kernel, rows_per_thread, z_chunks); the fused kernel is run in several launch geometries."""
     out = []
     with B.PoissonSolver(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, workspace=False) as s:
-        for v in (B.KERNEL_TWOPASS, B.KERNEL_RESIDENT, B.KERNEL_FUSED, B.KERNEL_FUSED_T2):
+        for v in (B.KERNEL_TWOPASS, B.KERNEL_RESIDENT, B.KERNEL_FUSED):
             try:
                 s.set_kernel(v)
             except B.PsError:
