@@ -367,8 +367,12 @@ int ps_set_fraction(ps_ctx *c, const double *F_dev, double rho_l, double rho_g)
     int rc = ensure_workspace(c);
     if (rc) return rc;
     const double cx = 1.0 / (c->dx * c->dx), cy = 1.0 / (c->dy * c->dy), cz = 1.0 / (c->dz * c->dz);
-    ps::ps_coef_build_kernel<<<grid_for(c, c->g.cells(), 256), 256, 0, c->stream>>>(
-        c->g, cx, cy, cz, rho_l, rho_g, F_dev, c->ax, c->ay, c->az);
+    if (c->g.nx % 2 == 0 && ((uintptr_t)F_dev & 15u) == 0)
+        ps::ps_coef_build_pair_kernel<<<grid_for(c, c->g.cells() / 2, 256), 256, 0, c->stream>>>(
+            c->g, cx, cy, cz, rho_l, rho_g, F_dev, c->ax, c->ay, c->az);
+    else
+        ps::ps_coef_build_kernel<<<grid_for(c, c->g.cells(), 256), 256, 0, c->stream>>>(
+            c->g, cx, cy, cz, rho_l, rho_g, F_dev, c->ax, c->ay, c->az);
     c->launches++;
     PS_CUDA(cudaGetLastError());
     c->have_coef = true;
