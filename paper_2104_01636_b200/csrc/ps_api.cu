@@ -218,8 +218,12 @@ int run_sweeps_untimed(ps_ctx *c, const double *rhs, double *p, double omega, in
 
 int enqueue_residual(ps_ctx *c, const double *rhs, const double *p, double tol)
 {
-    ps::ps_residual_partial_kernel<<<c->nparts, ps::RED_THREADS, 0, c->stream>>>(
-        c->g, c->ax, c->ay, c->az, rhs, p, c->partR2, c->partB2);
+    if (c->g.nx % 2 == 0 && (((uintptr_t)rhs | (uintptr_t)p) & 15u) == 0)
+        ps::ps_residual_partial_pair_kernel<<<c->nparts, ps::RED_THREADS, 0, c->stream>>>(
+            c->g, c->ax, c->ay, c->az, rhs, p, c->partR2, c->partB2);
+    else
+        ps::ps_residual_partial_kernel<<<c->nparts, ps::RED_THREADS, 0, c->stream>>>(
+            c->g, c->ax, c->ay, c->az, rhs, p, c->partR2, c->partB2);
     c->launches++;
     PS_CUDA(cudaGetLastError());
     ps::ps_reduce_final_kernel<<<1, ps::FIN_THREADS, 0, c->stream>>>(c->partR2, c->partB2,
@@ -549,8 +553,12 @@ int mg_launch_coarsen(ps_ctx *f, ps_ctx *k)
 
 int mg_launch_residual_restrict(ps_ctx *f, const double *rhs, const double *p, double *rc)
 {
-    ps::ps_mg_residual_restrict_kernel<<<grid_for(f, f->g.cells() / 8, 256), 256, 0, f->stream>>>(
-        f->g, f->ax, f->ay, f->az, rhs, p, rc);
+    if ((((uintptr_t)rhs | (uintptr_t)p) & 15u) == 0)
+        ps::ps_mg_residual_restrict_pair_kernel<<<grid_for(f, f->g.cells() / 8, 256), 256, 0,
+                                                  f->stream>>>(f->g, f->ax, f->ay, f->az, rhs, p, rc);
+    else
+        ps::ps_mg_residual_restrict_kernel<<<grid_for(f, f->g.cells() / 8, 256), 256, 0,
+                                             f->stream>>>(f->g, f->ax, f->ay, f->az, rhs, p, rc);
     f->launches++;
     PS_CUDA(cudaGetLastError());
     return PS_OK;

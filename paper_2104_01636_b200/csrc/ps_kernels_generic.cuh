@@ -156,6 +156,41 @@ __device__ __forceinline__ Stencil gather(const Grid &g, const double *__restric
     return s;
 }
 
+// Residuals of the x-pair of cells (n, n+1) (n even, nx even) with 16-byte loads; R returns the
+// rhs pair.  Same expression as residual_at(gather(...)) for each of the two cells.
+__device__ __forceinline__ double2 ld2(const double *q)
+{
+    return *reinterpret_cast<const double2 *>(q);
+}
+
+__device__ __forceinline__ double2 residual_pair(const Grid &g, const double *__restrict__ ax,
+                                                 const double *__restrict__ ay,
+                                                 const double *__restrict__ az,
+                                                 const double *__restrict__ rhs,
+                                                 const double *__restrict__ p, int i, int j, int k,
+                                                 size_t n, double2 &R)
+{
+    const size_t plane = (size_t)g.nx * g.ny;
+    const size_t nzm = (k > 0) ? n - plane : n + plane * (size_t)(g.nz - 1);
+    const size_t nzp = (k + 1 < g.nz) ? n + plane : n - plane * (size_t)(g.nz - 1);
+    const double2 P = ld2(p + n), AX = ld2(ax + n), AY = ld2(ay + n), AZ = ld2(az + n);
+    R = ld2(rhs + n);
+    const double axl = (i > 0) ? ax[n - 1] : 0.0;
+    const double2 AYm = (j > 0) ? ld2(ay + n - g.nx) : make_double2(0.0, 0.0);
+    const double2 AZm = ld2(az + nzm);
+    const double pl = p[(i > 0) ? n - 1 : n];
+    const double pr = p[(i + 2 < g.nx) ? n + 2 : n + 1];
+    const double2 Pym = ld2(p + ((j > 0) ? n - g.nx : n));
+    const double2 Pyp = ld2(p + ((j < g.ny - 1) ? n + g.nx : n));
+    const double2 Pzm = ld2(p + nzm), Pzp = ld2(p + nzp);
+    double2 r;
+    r.x = residual_at(axl, AX.x, AYm.x, AY.x, AZm.x, AZ.x, pl, P.y, Pym.x, Pyp.x, Pzm.x, Pzp.x, P.x,
+                      R.x);
+    r.y = residual_at(AX.x, AX.y, AYm.y, AY.y, AZm.y, AZ.y, P.x, pr, Pym.y, Pyp.y, Pzm.y, Pzp.y, P.y,
+                      R.y);
+    return r;
+}
+
 // Half-sweep, in place: one thread per cell of the active colour ((i+j+k)&1 == colour).
 // Cells of one colour never read each other, so no ordering between threads is needed.
 __global__ void __launch_bounds__(256)
@@ -242,6 +277,42 @@ ps_residual_partial_kernel(Grid g, const double *__restrict__ ax, const double *
     if (threadIdx.x == 0) {
         partR2[blockIdx.x] = R;
         partB2[blockIdx.x] = B;
+    }
+}
+
+// The same for even nx and 16-byte aligned rhs, p: thread t takes the x-pairs t, t+256, ... of the
+// block's chunk (left cell first).  A different but equally fixed summation tree.
+__global__ void __launch_bounds__(RED_THREADS)
+ps_residual_partial_pair_kernel(Grid g, const double *__restrict__ ax,
+                                const double *__restrict__ ay, const double *__restrict__ az,
+                                const double *__restrict__ rhs, const double *__restrict__ p,
+                                double *__restrict__ partR2, double *__restrict__ partB2)
+{
+    __shared__ double sm[RED_THREADS / 32];
+    const size_t N = g.cells();
+    const size_t base = (size_t)blockIdx.x * RED_CHUNK;
+    double r2 = 0.0, b2 = 0.0;
+#pragma unroll 2
+    for (int m = 0; m < RED_CHUNK / (2 * RED_THREADS); ++m) {
+        const size_t n = base + 2 * ((size_t)m * RED_THREADS + threadIdx.x);
+        if (n < N) {
+            const int i = (int)((unsigned)n % (unsigned)g.nx);
+            const unsigned t = (unsigned)n / (unsigned)g.nx;
+            const int j = (int)(t % (unsigned)g.ny);
+            const int k = (int)(t / (unsigned)g.ny);
+            double2 b;
+            const double2 r = residual_pair(g, ax, ay, az, rhs, p, i, j, k, n, b);
+            r2 = r2 + r.x * r.x;
+            r2 = r2 + r.y * r.y;
+            b2 = b2 + b.x * b.x;
+            b2 = b2 + b.y * b.y;
+        }
+    }
+    const double Rs = block_tree_sum<RED_THREADS>(r2, sm);
+    const double Bs = block_tree_sum<RED_THREADS>(b2, sm);
+    if (threadIdx.x == 0) {
+        partR2[blockIdx.x] = Rs;
+        partB2[blockIdx.x] = Bs;
     }
 }
 
