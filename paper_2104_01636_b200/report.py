@@ -67,6 +67,42 @@ def run_config(cfg: int, max_sweeps: int, to_tol: bool, kernel: int, mg_cycles: 
     return out
 
 
+def kernel_rates(cfg: int = 4, reps: int = 20) -> str:
+    """Per-kernel device time and algorithmic HBM rate of the single-pass kernels (DESIGN.md §7
+    bytes per cell), CUDA events around `reps` back-to-back launches each."""
+    import torch
+    from . import binding, workload as wl
+    w = wl.make_config(cfg)
+    F = torch.from_numpy(w.F).cuda()
+    u = [torch.randn(F.shape, dtype=torch.float64, device="cuda") for _ in range(3)]
+    p = torch.randn(F.shape, dtype=torch.float64, device="cuda")
+    kap = torch.rand(F.shape, dtype=torch.float64, device="cuda")
+    rhs = torch.empty_like(p)
+    rows = []
+    with binding.PoissonSolver(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz) as s:
+        s.set_fraction(F, w.rho_l, w.rho_g)
+        cases = [("ps_set_fraction (coefficient build)", lambda: s.set_fraction(F, w.rho_l, w.rho_g), 32),
+                 ("ps_residual (norm, incl. final reduction + read-back)", lambda: s.residual(rhs, p), 40),
+                 ("ps_mg_residual_restrict", lambda: s.mg_residual_restrict(rhs, p), 41),
+                 ("ps_rhs_from_velocity", lambda: s.rhs_from_velocity(*u, 1e-3, rhs), 32),
+                 ("ps_correct_velocity", lambda: s.correct_velocity(p, 1e-3, *u), 80),
+                 ("ps_face_divergence", lambda: s.face_divergence(*u, p, 1e-3), 64),
+                 ("ps_ssf_rhs", lambda: s.ssf_rhs(F, kap, 0.072), 48)]
+        for name, fn, nbytes in cases:
+            fn()
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(reps):
+                fn()
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / reps
+            rows.append(f"| `{name}` | {nbytes} | {ms * 1e3:.0f} | {w.cells * nbytes / ms / 1e6:.0f} |")
+    return ("| call (config %d, %d cells) | algorithmic B/cell | µs per call | GB/s |\n|---|---|---|---|\n"
+            % (cfg, w.cells)) + "\n".join(rows) + "\n"
+
+
 def to_markdown(rows) -> str:
     head = ("| cfg | workload | kernel | sweeps | ms | Gcell-upd/s | model GB/s | res_rel after | "
             "SOR to 1e-8: sweeps | seconds | res_rel | MG to 1e-8: cycles (levels) | seconds | res_rel |\n"
@@ -94,6 +130,8 @@ def main(argv=None):
     ap.add_argument("--sweeps", type=int, default=0, help="fixed-sweep count (default: the config's)")
     ap.add_argument("--kernel", default="auto", choices=["auto", "twopass", "fused"])
     ap.add_argument("--md", default="", help="also write the table to this file")
+    ap.add_argument("--kernel-rates", action="store_true",
+                    help="only time the single-pass kernels on config 4 and print their rates")
     args = ap.parse_args(argv)
     import torch
     from . import binding, build
@@ -103,6 +141,13 @@ def main(argv=None):
     binding.load()
     kernel = {"auto": binding.KERNEL_AUTO, "twopass": binding.KERNEL_TWOPASS,
               "fused": binding.KERNEL_FUSED}[args.kernel]
+    if args.kernel_rates:
+        md = kernel_rates()
+        print(md)
+        if args.md:
+            with open(args.md, "w") as f:
+                f.write(md)
+        return
     rows = []
     for cfg in [int(c) for c in args.configs.split(",")]:
         r = run_config(cfg, args.max_sweeps, to_tol=(not args.no_tol and str(cfg) in args.sor_tol_configs.split(',')), kernel=kernel,
