@@ -41,7 +41,8 @@ UNIT = "Gcell-updates/s"
 # algorithmic bytes per cell per sweep-kernel launch:
 #   twopass: one colour per launch, M1 = 40 B/cell/launch (80 B per cell-update)
 #   fused:   one sweep per launch,  M2 = 48 B/cell/launch (48 B per cell-update)
-ALGO_BYTES_PER_CELL_LAUNCH = {"twopass": 40.0, "fused": 48.0,
+#   fused_otf: the same with rho (8 B) in place of ax, ay, az (24 B) = 32 B per cell-update
+ALGO_BYTES_PER_CELL_LAUNCH = {"twopass": 40.0, "fused": 48.0, "fused_otf": 32.0,
                               "resident": 80.0}   # resident: L2-resident grids only, per sweep
 
 
@@ -54,7 +55,7 @@ def parse_args():
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json config 1..5 (default 4)")
     ap.add_argument("--sweeps", type=int, default=0, help="sweeps per step (default: the config's)")
     ap.add_argument("--kernel", default="auto",
-                    choices=["auto", "twopass", "fused", "resident"])
+                    choices=["auto", "twopass", "fused", "resident", "fused_otf"])
     ap.add_argument("--no-mg", action="store_true", help="skip the multigrid time-to-1e-8 leg")
     ap.add_argument("--rpt", type=int, default=0, help="fused kernel: rows per thread (0 = auto)")
     ap.add_argument("--zchunks", type=int, default=0, help="fused kernel: z chunks (0 = auto)")
@@ -225,7 +226,7 @@ def run_ours(args, rank):
     sweeps = sweeps_for(args.config, args.sweeps)
     shape = (w.nz, w.ny, w.nx)
     kernel = {"auto": binding.KERNEL_AUTO, "twopass": binding.KERNEL_TWOPASS,
-              "fused": binding.KERNEL_FUSED,
+              "fused": binding.KERNEL_FUSED, "fused_otf": binding.KERNEL_FUSED_OTF,
               "resident": binding.KERNEL_RESIDENT}[args.kernel]
 
     F_h = torch.from_numpy(w.F).pin_memory()

@@ -51,6 +51,12 @@ extern "C" {
                                /* temporally blocked in one launch), ping-pong p            */
 #define PS_KERNEL_RESIDENT 3   /* L2-resident grids: n sweeps in ONE cooperative launch,    */
                                /* grid-wide barrier per half-sweep, in place, any nx,ny>=1  */
+#define PS_KERNEL_FUSED_OTF 4  /* PS_KERNEL_FUSED with the face coefficients rebuilt in the  */
+                               /* sweep from a stored rho field (O2 evaluated on the fly:   */
+                               /* 32 instead of 48 B per cell-update, 8 more fp64 divisions */
+                               /* per pair of updates).  Select it    */
+                               /* BEFORE ps_set_fraction (which then also stores rho), else */
+                               /* the sweeps return PS_ESTATE.  64x16 boxes only.           */
 
 typedef struct ps_ctx ps_ctx;   /* opaque; one per grid */
 
@@ -89,7 +95,7 @@ int ps_set_stream(ps_ctx *c, void *cuda_stream);
 int ps_set_check_interval(ps_ctx *c, int K);
 
 /* Choose the sweep kernel (PS_KERNEL_*).  PS_EINVAL if the grid shape does not allow the
- * variant (the fused kernels need nx even). */
+ * variant (the fused kernels need nx even; PS_KERNEL_FUSED_OTF needs rows_per_thread = 1). */
 int ps_set_kernel(ps_ctx *c, int variant);
 int ps_get_kernel(const ps_ctx *c);          /* the variant AUTO resolved to, or the one set */
 

@@ -16,9 +16,9 @@ from dataclasses import dataclass
 from . import build as _build
 
 PS_OK, PS_EINVAL, PS_ESTATE, PS_ECUDA, PS_ENOMEM = 0, -1, -2, -3, -4
-KERNEL_AUTO, KERNEL_TWOPASS, KERNEL_FUSED, KERNEL_RESIDENT = 0, 1, 2, 3
+KERNEL_AUTO, KERNEL_TWOPASS, KERNEL_FUSED, KERNEL_RESIDENT, KERNEL_FUSED_OTF = 0, 1, 2, 3, 4
 KERNEL_NAMES = {KERNEL_AUTO: "auto", KERNEL_TWOPASS: "twopass", KERNEL_FUSED: "fused",
-                KERNEL_RESIDENT: "resident"}
+                KERNEL_RESIDENT: "resident", KERNEL_FUSED_OTF: "fused_otf"}
 
 # every symbol include/ps_poisson.h declares (tests check the library exports each one)
 SYMBOLS = ("ps_create", "ps_destroy", "ps_workspace_bytes", "ps_set_workspace", "ps_set_stream",

@@ -19,7 +19,7 @@ _CSRC = os.path.join(_HERE, "csrc")
 _INC = os.path.join(os.path.dirname(_HERE), "include")
 LIB = os.path.join(_HERE, "libps_poisson.so")
 SOURCES = ["ps_api.cu"]
-HEADERS = ["ps_kernels_generic.cuh", "ps_kernels_zmarch.cuh"]
+HEADERS = sorted(f for f in os.listdir(_CSRC) if f.endswith(".cuh"))
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

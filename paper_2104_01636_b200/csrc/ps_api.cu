@@ -47,6 +47,7 @@ struct ps_ctx {
     int variant_req;       // what the caller asked for (PS_KERNEL_*)
     int variant;           // resolved
     bool have_coef;
+    bool have_rho;         // rho field of the on-the-fly sweep variant is current
     int sm_count;
     int coop;              // device supports cooperative launches
     long long launches;
@@ -54,7 +55,7 @@ struct ps_ctx {
     void *ws;
     size_t ws_bytes;
     bool ws_owned;
-    double *ax, *ay, *az, *p_alt, *partR2, *partB2, *scal;   // scal: 3 doubles out
+    double *ax, *ay, *az, *p_alt, *rho, *partR2, *partB2, *scal;   // scal: 3 doubles out
     int *done;
     int nparts;
     double *h_scal;        // pinned, 4 doubles
@@ -81,7 +82,7 @@ size_t field_bytes(const ps_ctx *c) { return align_up(c->g.cells() * sizeof(doub
 
 size_t workspace_bytes(const ps_ctx *c)
 {
-    return 4 * field_bytes(c) + 2 * align_up((size_t)c->nparts * sizeof(double), 256) + 256 + 256;
+    return 5 * field_bytes(c) + 2 * align_up((size_t)c->nparts * sizeof(double), 256) + 256 + 256;
 }
 
 void carve(ps_ctx *c, void *base)
@@ -92,6 +93,7 @@ void carve(ps_ctx *c, void *base)
     c->ay = (double *)q; q += fb;
     c->az = (double *)q; q += fb;
     c->p_alt = (double *)q; q += fb;
+    c->rho = (double *)q; q += fb;
     c->partR2 = (double *)q; q += pb;
     c->partB2 = (double *)q; q += pb;
     c->scal = (double *)q; q += 256;
@@ -121,8 +123,9 @@ int resolve_variant(const ps_ctx *c, int req)
         return PS_KERNEL_RESIDENT;
     if (req == PS_KERNEL_AUTO) return fused_ok ? PS_KERNEL_FUSED : PS_KERNEL_TWOPASS;
     if (req == PS_KERNEL_FUSED && !fused_ok) return -1;
+    if (req == PS_KERNEL_FUSED_OTF && !(fused_ok && c->fused.rpt == 1)) return -1;
     if (req == PS_KERNEL_RESIDENT && !c->coop) return -1;
-    if (req < PS_KERNEL_AUTO || req > PS_KERNEL_RESIDENT) return -1;
+    if (req < PS_KERNEL_AUTO || req > PS_KERNEL_FUSED_OTF) return -1;
     return req;
 }
 
@@ -201,9 +204,16 @@ int run_sweeps_untimed(ps_ctx *c, const double *rhs, double *p, double omega, in
     }
     double *src = p, *dst = c->p_alt;
     int left = n;
+    const bool otf = c->variant == PS_KERNEL_FUSED_OTF;
+    if (otf && !c->have_rho) return PS_ESTATE;
+    const double c2x = 2.0 * (1.0 / (c->dx * c->dx)), c2y = 2.0 * (1.0 / (c->dy * c->dy)),
+                 c2z = 2.0 * (1.0 / (c->dz * c->dz));
     while (left > 0) {
-        cudaError_t e = ps::zm_launch(c->fused, c->g, c->ax, c->ay, c->az, rhs, src, dst, omega,
-                                      c->stream);
+        cudaError_t e =
+            otf ? ps::zm_launch_otf(c->fused, c->g, c->rho, c2x, c2y, c2z, rhs, src, dst, omega,
+                                    c->stream)
+                : ps::zm_launch(c->fused, c->g, c->ax, c->ay, c->az, rhs, src, dst, omega,
+                                c->stream);
         c->launches++;
         if (e != cudaSuccess) return cuda_fail(e);
         left -= 1;
@@ -311,6 +321,7 @@ int ps_set_workspace(ps_ctx *c, void *ws_dev, size_t bytes)
     c->ws_bytes = bytes;
     c->ws_owned = false;
     c->have_coef = false;
+    c->have_rho = false;
     carve(c, ws_dev);
     return PS_OK;
 }
@@ -347,6 +358,7 @@ int ps_set_tuning(ps_ctx *c, int rows_per_thread, int z_chunks)
     if (rows_per_thread < 0 || rows_per_thread > 2 || z_chunks < 0 || z_chunks > c->g.nz / 2)
         return PS_EINVAL;
     const int rpt = rows_per_thread ? rows_per_thread : c->fused.rpt;
+    if (c->variant == PS_KERNEL_FUSED_OTF && rpt != 1) return PS_EINVAL;
     PS_CUDA(cudaStreamSynchronize(c->stream));
     const cudaError_t e = ps::zm_plan_tiles(&c->fused, c->g, rpt, z_chunks);
     if (e == cudaErrorInvalidValue) { cudaGetLastError(); return PS_EINVAL; }
@@ -379,6 +391,14 @@ int ps_set_fraction(ps_ctx *c, const double *F_dev, double rho_l, double rho_g)
             c->g, cx, cy, cz, rho_l, rho_g, F_dev, c->ax, c->ay, c->az);
     c->launches++;
     PS_CUDA(cudaGetLastError());
+    c->have_rho = false;
+    if (c->variant == PS_KERNEL_FUSED_OTF) {
+        ps::ps_rho_build_kernel<<<grid_for(c, c->g.cells(), 256), 256, 0, c->stream>>>(
+            c->g.cells(), rho_l, rho_g, F_dev, c->rho);
+        c->launches++;
+        PS_CUDA(cudaGetLastError());
+        c->have_rho = true;
+    }
     c->have_coef = true;
     c->mg_ready = false;
     return PS_OK;

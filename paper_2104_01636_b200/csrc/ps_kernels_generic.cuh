@@ -125,6 +125,19 @@ ps_coef_build_pair_kernel(Grid g, double cx, double cy, double cz, double rho_l,
     }
 }
 
+// O1 alone: rho = rho_l F + rho_g (1 - F), kept for the sweep variant that rebuilds the face
+// coefficients on the fly (PS_KERNEL_FUSED_OTF).  8 B in, 8 B out per cell.
+__global__ void __launch_bounds__(256)
+ps_rho_build_kernel(size_t N, double rho_l, double rho_g, const double *__restrict__ F,
+                    double *__restrict__ rho)
+{
+    for (size_t n = (size_t)blockIdx.x * blockDim.x + threadIdx.x; n < N;
+         n += (size_t)gridDim.x * blockDim.x) {
+        const double Fc = F[n];
+        rho[n] = (rho_l * Fc) + (rho_g * (1.0 - Fc));
+    }
+}
+
 // ---------------------------------------------------------------------------------------------
 // Gather the six coefficients and neighbour values of cell (i,j,k) from natural-layout arrays.
 // Wall neighbours are read at the clamped index (a finite number) and meet a 0.0 coefficient.

@@ -47,7 +47,8 @@ def variants_for(B, w, tunings=((1, 0), (2, 0), (1, 1), (2, 3))):
     (kernel, rows_per_thread, z_chunks); the fused kernel is run in several launch geometries."""
     out = []
     with B.PoissonSolver(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, workspace=False) as s:
-        for v in (B.KERNEL_TWOPASS, B.KERNEL_RESIDENT, B.KERNEL_FUSED):
+        # FUSED_OTF before FUSED: it only takes 16-row boxes and the tunings below end on 32
+        for v in (B.KERNEL_TWOPASS, B.KERNEL_RESIDENT, B.KERNEL_FUSED_OTF, B.KERNEL_FUSED):
             try:
                 s.set_kernel(v)
             except B.PsError:
@@ -344,3 +345,32 @@ def test_non_default_stream_and_library_workspace(torch_cuda, B, ora):
     st.synchronize()
     assert_p_parity(p_d.cpu().numpy(), p_ora, "side stream")
     s.close()
+
+
+# ---------------------------------------------------------------- NEXT-4: on-the-fly coefficients
+@pytest.mark.parametrize("shape", [(40, 36, 24, 2, 8, None), (72, 52, 34, 3, 12, (1 / 72, 1 / 60, 1 / 50)),
+                                   (132, 20, 10, 0, 0, None), (64, 16, 8, 0, 0, None),
+                                   (2, 1, 2, 0, 0, None)])
+def test_on_the_fly_coefficients_bitwise(torch_cuda, B, ora, shape):
+    """PS_KERNEL_FUSED_OTF rebuilds ax, ay, az from rho inside the sweep:
+    p must equal the oracle's (which sweeps with stored O2 coefficients) to the last bit, and the
+    variant must be chosen before ps_set_fraction (PS_ESTATE otherwise)."""
+    w = shape_workload(*shape)
+    coef = ora.coefficients(w.F, w.rho_l, w.rho_g, w.dx, w.dy, w.dz)
+    p_ora = np.zeros_like(w.rhs)
+    ora.sweep(coef, w.rhs, p_ora, w.omega, 7)
+    F_d, rhs_d = to_dev(torch_cuda, w.F), to_dev(torch_cuda, w.rhs)
+    with B.PoissonSolver(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz) as s:
+        s.set_fraction(F_d, w.rho_l, w.rho_g)
+        s.set_kernel(B.KERNEL_FUSED_OTF)
+        p_d = torch_cuda.zeros_like(rhs_d)
+        with pytest.raises(B.PsError) as e:
+            s.sweeps(rhs_d, p_d, w.omega, 1)          # rho was not stored by that set_fraction
+        assert e.value.code == B.PS_ESTATE
+        with pytest.raises(B.PsError):
+            s.set_tuning(2, 0)                        # 16-row boxes only
+        s.set_fraction(F_d, w.rho_l, w.rho_g)
+        s.sweeps(rhs_d, p_d, w.omega, 7)
+        assert_p_parity(p_d.cpu().numpy(), p_ora, "fused_otf x7")
+        info = s.solve(rhs_d, p_d, w.omega, 0, 0.0)   # norms still come from the stored coefficients
+        assert abs(info.res_rel - ora.residual(coef, w.rhs, p_ora)[1]) <= NORM_TOL * info.res_rel
