@@ -56,7 +56,7 @@ extern "C" {
                                /* 32 instead of 48 B per cell-update, 8 more fp64 divisions */
                                /* per pair of updates).  Select it    */
                                /* BEFORE ps_set_fraction (which then also stores rho), else */
-                               /* the sweeps return PS_ESTATE.  64x16 boxes only.           */
+                               /* the sweeps return PS_ESTATE.                              */
 
 typedef struct ps_ctx ps_ctx;   /* opaque; one per grid */
 
@@ -95,12 +95,12 @@ int ps_set_stream(ps_ctx *c, void *cuda_stream);
 int ps_set_check_interval(ps_ctx *c, int K);
 
 /* Choose the sweep kernel (PS_KERNEL_*).  PS_EINVAL if the grid shape does not allow the
- * variant (the fused kernels need nx even; PS_KERNEL_FUSED_OTF needs rows_per_thread = 1). */
+ * variant (the fused kernels need nx even). */
 int ps_set_kernel(ps_ctx *c, int variant);
 int ps_get_kernel(const ps_ctx *c);          /* the variant AUTO resolved to, or the one set */
 
 /* Launch geometry of the fused kernel (tuning and tests; every setting gives bitwise identical p).
- * rows_per_thread: 1 = 64x16-cell boxes, 2 = 64x32-cell boxes, 0 = keep.  z_chunks: number of
+ * rows_per_thread: 1 = 64x16-cell boxes (the only height built), 0 = keep.  z_chunks: number of
  * z chunks each (x,y) tile is cut into (CTAs = tiles * z_chunks), 0 = choose by the cost model
  * (rounds of sm_count CTAs x (planes per chunk + z halo)).  Synchronises the stream.
  * PS_EINVAL: fused kernel not available for this grid, values out of range. */
