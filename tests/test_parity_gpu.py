@@ -373,3 +373,62 @@ def test_on_the_fly_coefficients_bitwise(torch_cuda, B, ora, shape):
         assert_p_parity(p_d.cpu().numpy(), p_ora, "fused_otf x7")
         info = s.solve(rhs_d, p_d, w.omega, 0, 0.0)   # norms still come from the stored coefficients
         assert abs(info.res_rel - ora.residual(coef, w.rhs, p_ora)[1]) <= NORM_TOL * info.res_rel
+
+
+# ---------------------------------------------------------------- tile-geometry edge cases
+@pytest.mark.parametrize("nx,ny,nz", [
+    (64, 16, 4),      # exactly one box: both walls of x and of y inside one tile
+    (66, 17, 4),      # one cell / one row more than a box: two tiles each way
+    (62, 30, 6),      # two wall tiles of the maximum height (15 rows each)
+    (124, 31, 4),     # 62 + 62 columns; 15 + 16 rows -> three row tiles
+    (126, 44, 4),     # needs a middle tile in x; 15 + 14 + 15 rows
+    (186, 45, 6),     # 62 + 60 + 62 (+2) columns; one row more than 15 + 14 + 15
+    (2, 2, 2),        # smallest grid the fused kernels take
+])
+def test_fused_tile_edges_bitwise(torch_cuda, B, ora, nx, ny, nz):
+    """Fused kernels (stored and on-the-fly coefficients) on grids whose sizes sit on the tile
+    capacities of the 64-column x 16-row box (62 / 60 columns, 15 / 14 rows per wall / middle
+    tile), with 1 and 2 z chunks: p bitwise equal to the oracle after 3 sweeps."""
+    w = shape_workload(nx, ny, nz, 0, 0, None, seed=nx + ny)
+    coef = ora.coefficients(w.F, w.rho_l, w.rho_g, w.dx, w.dy, w.dz)
+    p0 = wl.noise_rhs(w.nx, w.ny, w.nz, 5)
+    p_ora = p0.copy()
+    ora.sweep(coef, w.rhs, p_ora, w.omega, 3)
+    for kernel in (B.KERNEL_FUSED, B.KERNEL_FUSED_OTF):
+        for chunks in (1, 2):
+            if chunks > nz // 2:
+                continue
+            with B.PoissonSolver(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz) as s:
+                s.set_kernel(kernel)
+                s.set_tuning(1, chunks)
+                s.set_fraction(to_dev(torch_cuda, w.F), w.rho_l, w.rho_g)
+                p_d = to_dev(torch_cuda, p0)
+                s.sweeps(to_dev(torch_cuda, w.rhs), p_d, w.omega, 3)
+                assert_p_parity(p_d.cpu().numpy(), p_ora, f"{nx}x{ny}x{nz} kernel {kernel} chunks {chunks}")
+
+
+def test_wide_dynamic_range_bitwise(torch_cuda, B, ora):
+    """IEEE division and rounding outside the comfortable range: |rhs| = 2^k with k drawn from
+    [-1070, 400] (subnormal numerators up to huge ones) sends many quotients of the update through
+    the GPU's division slow path; every variant must still equal the host's correctly rounded
+    arithmetic bit for bit."""
+    nx, ny, nz = 40, 36, 24
+    w = shape_workload(nx, ny, nz, 2, 8, None)
+    rng = np.random.default_rng(2104)
+    k = rng.integers(-1070, 401, size=(nz, ny, nx))
+    rhs = np.ldexp(rng.choice([-1.0, 1.0], size=k.shape), k)
+    assert np.isfinite(rhs).all() and (np.abs(rhs[rhs != 0]) < 2.3e-308).any()   # has subnormals
+    coef = ora.coefficients(w.F, w.rho_l, w.rho_g, w.dx, w.dy, w.dz)
+    for nsweeps in (1, 2):                        # after 1 sweep red cells still hold subnormals
+        p_ora = np.zeros_like(rhs)
+        ora.sweep(coef, rhs, p_ora, w.omega, nsweeps)
+        assert np.isfinite(p_ora).all()
+        if nsweeps == 1:
+            assert np.count_nonzero((np.abs(p_ora) < 2.3e-308) & (p_ora != 0)) > 100
+        for variant in variants_for(B, w):
+            with make_solver(B, w, variant) as s:
+                s.set_fraction(to_dev(torch_cuda, w.F), w.rho_l, w.rho_g)
+                p_d = torch_cuda.zeros(nz, ny, nx, dtype=torch_cuda.float64, device="cuda")
+                s.sweeps(to_dev(torch_cuda, rhs), p_d, w.omega, nsweeps)
+                p_gpu = p_d.cpu().numpy()
+                assert int(np.count_nonzero(p_gpu != p_ora)) == 0, f"variant {variant} x{nsweeps}"
