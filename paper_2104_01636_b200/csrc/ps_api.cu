@@ -37,6 +37,13 @@ constexpr size_t ps_resident_max_cells = 131072;
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
+// all pointers 16-byte aligned (the pair kernels use 16-byte loads and stores)
+bool aligned16(const void *a, const void *b = nullptr, const void *c = nullptr,
+               const void *d = nullptr)
+{
+    return (((uintptr_t)a | (uintptr_t)b | (uintptr_t)c | (uintptr_t)d) & 15u) == 0;
+}
+
 }  // namespace
 
 struct ps_ctx {
@@ -728,8 +735,13 @@ int ps_rhs_from_velocity(ps_ctx *c, const double *ux_dev, const double *uy_dev,
     if (!c || !ux_dev || !uy_dev || !uz_dev || !rhs_dev) return PS_EINVAL;
     if (!(dt > 0.0) || !std::isfinite(dt)) return PS_EINVAL;
     const ps::Spacing h{c->dx, c->dy, c->dz};
-    ps::ps_rhs_from_velocity_kernel<<<grid_for(c, c->g.cells(), 256), 256, 0, c->stream>>>(
-        c->g, h, ux_dev, uy_dev, uz_dev, dt, rhs_dev);
+    if (c->g.nx % 2 == 0 && aligned16(ux_dev, uy_dev, uz_dev, rhs_dev))
+        ps::ps_rhs_from_velocity_pair_kernel<<<grid_for(c, c->g.cells() / 2, 256), 256, 0,
+                                               c->stream>>>(c->g, h, ux_dev, uy_dev, uz_dev, dt,
+                                                            rhs_dev);
+    else
+        ps::ps_rhs_from_velocity_kernel<<<grid_for(c, c->g.cells(), 256), 256, 0, c->stream>>>(
+            c->g, h, ux_dev, uy_dev, uz_dev, dt, rhs_dev);
     c->launches++;
     PS_CUDA(cudaGetLastError());
     return PS_OK;
@@ -756,8 +768,13 @@ int ps_face_divergence(ps_ctx *c, const double *ux_dev, const double *uy_dev, co
     if (!(dt > 0.0) || !std::isfinite(dt)) return PS_EINVAL;
     if (!c->have_coef) return PS_ESTATE;
     const ps::Spacing h{c->dx, c->dy, c->dz};
-    ps::ps_face_divergence_kernel<<<grid_for(c, c->g.cells(), 256), 256, 0, c->stream>>>(
-        c->g, h, c->ax, c->ay, c->az, ux_dev, uy_dev, uz_dev, p_dev, dt, div_dev);
+    if (c->g.nx % 2 == 0 && aligned16(ux_dev, uy_dev, uz_dev, p_dev) && aligned16(div_dev))
+        ps::ps_face_divergence_pair_kernel<<<grid_for(c, c->g.cells() / 2, 256), 256, 0,
+                                             c->stream>>>(c->g, h, c->ax, c->ay, c->az, ux_dev,
+                                                          uy_dev, uz_dev, p_dev, dt, div_dev);
+    else
+        ps::ps_face_divergence_kernel<<<grid_for(c, c->g.cells(), 256), 256, 0, c->stream>>>(
+            c->g, h, c->ax, c->ay, c->az, ux_dev, uy_dev, uz_dev, p_dev, dt, div_dev);
     c->launches++;
     PS_CUDA(cudaGetLastError());
     return PS_OK;
@@ -768,8 +785,12 @@ int ps_ssf_rhs(ps_ctx *c, const double *F_dev, const double *kappa_dev, double s
 {
     if (!c || !F_dev || !kappa_dev || !rhs_dev || !std::isfinite(sigma)) return PS_EINVAL;
     if (!c->have_coef) return PS_ESTATE;
-    ps::ps_ssf_rhs_kernel<<<grid_for(c, c->g.cells(), 256), 256, 0, c->stream>>>(
-        c->g, c->ax, c->ay, c->az, F_dev, kappa_dev, sigma, rhs_dev);
+    if (c->g.nx % 2 == 0 && aligned16(F_dev, kappa_dev, rhs_dev))
+        ps::ps_ssf_rhs_pair_kernel<<<grid_for(c, c->g.cells() / 2, 256), 256, 0, c->stream>>>(
+            c->g, c->ax, c->ay, c->az, F_dev, kappa_dev, sigma, rhs_dev);
+    else
+        ps::ps_ssf_rhs_kernel<<<grid_for(c, c->g.cells(), 256), 256, 0, c->stream>>>(
+            c->g, c->ax, c->ay, c->az, F_dev, kappa_dev, sigma, rhs_dev);
     c->launches++;
     PS_CUDA(cudaGetLastError());
     return PS_OK;

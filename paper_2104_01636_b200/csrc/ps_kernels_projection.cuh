@@ -5,7 +5,7 @@
 //   ps_correct_velocity_kernel    u_c <- u^_c - dt (grad p/rho)_{f->c}
 //   ps_face_divergence_kernel     div(u^_f - dt (grad p/rho)_f)   (= dt (rhs - A p))
 //
-// Single-pass streaming kernels, one thread per cell, natural layout, neighbour reuse through
+// single-pass streaming kernels, one thread per cell (per x-pair of cells for even nx), natural layout, neighbour reuse through
 // L1/L2; HBM-bound: 32 B/cell (rhs), 80 B/cell (correction: p 8, coefficients 24, u 24 + 24),
 // 64 B/cell (face divergence).  Expression order = the oracle's (compile with --fmad=false).
 #pragma once
@@ -117,6 +117,127 @@ ps_face_divergence_kernel(Grid g, Spacing h, const double *__restrict__ ax,
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// The same three-field stencils for even nx and 16-byte aligned arrays: one thread per x-pair of
+// cells (n, n+1), 16-byte loads and stores, 32-bit pair index.  Every value is produced by the
+// same expression as in the one-cell kernels above.
+struct PairCell { int i, j, k; size_t n, nzm, nzp; };
+
+__device__ __forceinline__ PairCell pair_cell(const Grid &g, unsigned h)
+{
+    const unsigned hx = (unsigned)g.nx >> 1;
+    PairCell c;
+    c.i = 2 * (int)(h % hx);
+    const unsigned t = h / hx;
+    c.j = (int)(t % (unsigned)g.ny);
+    c.k = (int)(t / (unsigned)g.ny);
+    c.n = g.idx(c.i, c.j, c.k);
+    const size_t plane = (size_t)g.nx * g.ny;
+    c.nzm = (c.k > 0) ? c.n - plane : c.n + plane * (size_t)(g.nz - 1);
+    c.nzp = (c.k + 1 < g.nz) ? c.n + plane : c.n - plane * (size_t)(g.nz - 1);
+    return c;
+}
+
+// fa[0..5], fb[0..5]: face velocities of the left and the right cell of the pair.
+__device__ __forceinline__ void face_velocities_pair(const Grid &g, const double *__restrict__ ux,
+                                                     const double *__restrict__ uy,
+                                                     const double *__restrict__ uz,
+                                                     const PairCell &c, double fa[6], double fb[6])
+{
+    const double2 UX = ld2(ux + c.n), UY = ld2(uy + c.n), UZ = ld2(uz + c.n);
+    const double2 UZm = ld2(uz + c.nzm), UZp = ld2(uz + c.nzp);
+    const double mid = 0.5 * (UX.x + UX.y);
+    fa[0] = (c.i > 0) ? 0.5 * (ux[c.n - 1] + UX.x) : 0.0;
+    fa[1] = mid;
+    fb[0] = mid;
+    fb[1] = (c.i + 2 < g.nx) ? 0.5 * (UX.y + ux[c.n + 2]) : 0.0;
+    fa[2] = fb[2] = fa[3] = fb[3] = 0.0;
+    if (c.j > 0) {
+        const double2 U = ld2(uy + c.n - g.nx);
+        fa[2] = 0.5 * (U.x + UY.x);
+        fb[2] = 0.5 * (U.y + UY.y);
+    }
+    if (c.j < g.ny - 1) {
+        const double2 U = ld2(uy + c.n + g.nx);
+        fa[3] = 0.5 * (UY.x + U.x);
+        fb[3] = 0.5 * (UY.y + U.y);
+    }
+    fa[4] = 0.5 * (UZm.x + UZ.x);
+    fb[4] = 0.5 * (UZm.y + UZ.y);
+    fa[5] = 0.5 * (UZ.x + UZp.x);
+    fb[5] = 0.5 * (UZ.y + UZp.y);
+}
+
+// ga[0..5], gb[0..5]: (grad p / rho) . n on the faces of the two cells (face_gradients per cell).
+__device__ __forceinline__ void face_gradients_pair(const Grid &g, const Spacing &h,
+                                                    const double *__restrict__ ax,
+                                                    const double *__restrict__ ay,
+                                                    const double *__restrict__ az,
+                                                    const double *__restrict__ p, const PairCell &c,
+                                                    double ga[6], double gb[6])
+{
+    const double2 P = ld2(p + c.n), AX = ld2(ax + c.n), AY = ld2(ay + c.n), AZ = ld2(az + c.n);
+    const double2 AZm = ld2(az + c.nzm), Pzm = ld2(p + c.nzm), Pzp = ld2(p + c.nzp);
+    const double axl = (c.i > 0) ? ax[c.n - 1] : 0.0;
+    const double pl = p[(c.i > 0) ? c.n - 1 : c.n];
+    const double pr = p[(c.i + 2 < g.nx) ? c.n + 2 : c.n + 1];
+    const double2 AYm = (c.j > 0) ? ld2(ay + c.n - g.nx) : make_double2(0.0, 0.0);
+    const double2 Pym = ld2(p + ((c.j > 0) ? c.n - g.nx : c.n));
+    const double2 Pyp = ld2(p + ((c.j < g.ny - 1) ? c.n + g.nx : c.n));
+    ga[0] = (axl * h.dx) * (P.x - pl);
+    ga[1] = (AX.x * h.dx) * (P.y - P.x);
+    gb[0] = (AX.x * h.dx) * (P.y - P.x);
+    gb[1] = (AX.y * h.dx) * (pr - P.y);
+    ga[2] = (AYm.x * h.dy) * (P.x - Pym.x);
+    gb[2] = (AYm.y * h.dy) * (P.y - Pym.y);
+    ga[3] = (AY.x * h.dy) * (Pyp.x - P.x);
+    gb[3] = (AY.y * h.dy) * (Pyp.y - P.y);
+    ga[4] = (AZm.x * h.dz) * (P.x - Pzm.x);
+    gb[4] = (AZm.y * h.dz) * (P.y - Pzm.y);
+    ga[5] = (AZ.x * h.dz) * (Pzp.x - P.x);
+    gb[5] = (AZ.y * h.dz) * (Pzp.y - P.y);
+}
+
+__global__ void __launch_bounds__(256)
+ps_rhs_from_velocity_pair_kernel(Grid g, Spacing h, const double *__restrict__ ux,
+                                 const double *__restrict__ uy, const double *__restrict__ uz,
+                                 double dt, double *__restrict__ rhs)
+{
+    const unsigned pairs = ((unsigned)g.nx >> 1) * (unsigned)g.ny * (unsigned)g.nz;
+    for (unsigned q = blockIdx.x * blockDim.x + threadIdx.x; q < pairs; q += gridDim.x * blockDim.x) {
+        const PairCell c = pair_cell(g, q);
+        double fa[6], fb[6];
+        face_velocities_pair(g, ux, uy, uz, c, fa, fb);
+        const double da = (((fa[1] - fa[0]) / h.dx) + ((fa[3] - fa[2]) / h.dy)) + ((fa[5] - fa[4]) / h.dz);
+        const double db = (((fb[1] - fb[0]) / h.dx) + ((fb[3] - fb[2]) / h.dy)) + ((fb[5] - fb[4]) / h.dz);
+        *reinterpret_cast<double2 *>(rhs + c.n) = make_double2(da / dt, db / dt);
+    }
+}
+
+__global__ void __launch_bounds__(256)
+ps_face_divergence_pair_kernel(Grid g, Spacing h, const double *__restrict__ ax,
+                               const double *__restrict__ ay, const double *__restrict__ az,
+                               const double *__restrict__ ux, const double *__restrict__ uy,
+                               const double *__restrict__ uz, const double *__restrict__ p,
+                               double dt, double *__restrict__ div)
+{
+    const unsigned pairs = ((unsigned)g.nx >> 1) * (unsigned)g.ny * (unsigned)g.nz;
+    for (unsigned q = blockIdx.x * blockDim.x + threadIdx.x; q < pairs; q += gridDim.x * blockDim.x) {
+        const PairCell c = pair_cell(g, q);
+        double fa[6], fb[6], ga[6], gb[6], ua[6], ub[6];
+        face_velocities_pair(g, ux, uy, uz, c, fa, fb);
+        face_gradients_pair(g, h, ax, ay, az, p, c, ga, gb);
+#pragma unroll
+        for (int m = 0; m < 6; ++m) {
+            ua[m] = fa[m] - dt * ga[m];
+            ub[m] = fb[m] - dt * gb[m];
+        }
+        const double da = (((ua[1] - ua[0]) / h.dx) + ((ua[3] - ua[2]) / h.dy)) + ((ua[5] - ua[4]) / h.dz);
+        const double db = (((ub[1] - ub[0]) / h.dx) + ((ub[3] - ub[2]) / h.dy)) + ((ub[5] - ub[4]) / h.dz);
+        *reinterpret_cast<double2 *>(div + c.n) = make_double2(da, db);
+    }
+}
+
 }  // namespace ps
 
 // ---------------------------------------------------------------------------------------------
@@ -150,6 +271,57 @@ ps_ssf_rhs_kernel(Grid g, const double *__restrict__ ax, const double *__restric
             t[q] = (a[q] * (sigma * kf)) * (F[nb[q]] - Fc);
         }
         rhs[n] = -(((((t[0] + t[1]) + t[2]) + t[3]) + t[4]) + t[5]);
+    }
+}
+
+// One thread per x-pair (even nx, 16-byte aligned arrays); the same expressions per cell.
+__device__ __forceinline__ double ssf_term(double a, double sigma, double kc, double kn, double Fc,
+                                           double Fn)
+{
+    const double kf = 0.5 * (kc + kn);
+    return (a * (sigma * kf)) * (Fn - Fc);
+}
+
+__global__ void __launch_bounds__(256)
+ps_ssf_rhs_pair_kernel(Grid g, const double *__restrict__ ax, const double *__restrict__ ay,
+                       const double *__restrict__ az, const double *__restrict__ F,
+                       const double *__restrict__ kappa, double sigma, double *__restrict__ rhs)
+{
+    const unsigned pairs = ((unsigned)g.nx >> 1) * (unsigned)g.ny * (unsigned)g.nz;
+    for (unsigned q = blockIdx.x * blockDim.x + threadIdx.x; q < pairs; q += gridDim.x * blockDim.x) {
+        const PairCell c = pair_cell(g, q);
+        const size_t n = c.n;
+        const double2 Fc = ld2(F + n), Kc = ld2(kappa + n);
+        const double2 AX = ld2(ax + n), AY = ld2(ay + n), AZ = ld2(az + n), AZm = ld2(az + c.nzm);
+        const double axl = (c.i > 0) ? ax[n - 1] : 0.0;
+        const size_t nl = (c.i > 0) ? n - 1 : n, nr = (c.i + 2 < g.nx) ? n + 2 : n + 1;
+        const size_t nym = (c.j > 0) ? n - g.nx : n, nyp = (c.j < g.ny - 1) ? n + g.nx : n;
+        const double2 AYm = (c.j > 0) ? ld2(ay + nym) : make_double2(0.0, 0.0);
+        const double Fl = F[nl], Kl = kappa[nl], Fr = F[nr], Kr = kappa[nr];
+        const double2 Fym = ld2(F + nym), Kym = ld2(kappa + nym), Fyp = ld2(F + nyp),
+                      Kyp = ld2(kappa + nyp);
+        const double2 Fzm = ld2(F + c.nzm), Kzm = ld2(kappa + c.nzm), Fzp = ld2(F + c.nzp),
+                      Kzp = ld2(kappa + c.nzp);
+        double2 out;
+        {   // left cell (i): x- neighbour nl, x+ neighbour the right cell
+            const double t0 = ssf_term(axl, sigma, Kc.x, Kl, Fc.x, Fl);
+            const double t1 = ssf_term(AX.x, sigma, Kc.x, Kc.y, Fc.x, Fc.y);
+            const double t2 = ssf_term(AYm.x, sigma, Kc.x, Kym.x, Fc.x, Fym.x);
+            const double t3 = ssf_term(AY.x, sigma, Kc.x, Kyp.x, Fc.x, Fyp.x);
+            const double t4 = ssf_term(AZm.x, sigma, Kc.x, Kzm.x, Fc.x, Fzm.x);
+            const double t5 = ssf_term(AZ.x, sigma, Kc.x, Kzp.x, Fc.x, Fzp.x);
+            out.x = -(((((t0 + t1) + t2) + t3) + t4) + t5);
+        }
+        {   // right cell (i+1): x- neighbour the left cell, x+ neighbour nr (itself at the wall)
+            const double t0 = ssf_term(AX.x, sigma, Kc.y, Kc.x, Fc.y, Fc.x);
+            const double t1 = ssf_term(AX.y, sigma, Kc.y, Kr, Fc.y, Fr);
+            const double t2 = ssf_term(AYm.y, sigma, Kc.y, Kym.y, Fc.y, Fym.y);
+            const double t3 = ssf_term(AY.y, sigma, Kc.y, Kyp.y, Fc.y, Fyp.y);
+            const double t4 = ssf_term(AZm.y, sigma, Kc.y, Kzm.y, Fc.y, Fzm.y);
+            const double t5 = ssf_term(AZ.y, sigma, Kc.y, Kzp.y, Fc.y, Fzp.y);
+            out.y = -(((((t0 + t1) + t2) + t3) + t4) + t5);
+        }
+        *reinterpret_cast<double2 *>(rhs + n) = out;
     }
 }
 
