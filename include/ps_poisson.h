@@ -100,7 +100,8 @@ int ps_set_kernel(ps_ctx *c, int variant);
 int ps_get_kernel(const ps_ctx *c);          /* the variant AUTO resolved to, or the one set */
 
 /* Launch geometry of the fused kernel (tuning and tests; every setting gives bitwise identical p).
- * rows_per_thread: 1 = 64x16-cell boxes (the only height built), 0 = keep.  z_chunks: number of
+ * rows_per_thread: rows of the 64x16-cell box one thread updates per step: 1 = 16 compute warps
+ * (default, fastest on B200), 2 = 8 compute warps with two rows each, 0 = keep.  z_chunks: number of
  * z chunks each (x,y) tile is cut into (CTAs = tiles * z_chunks), 0 = choose by the cost model
  * (rounds of sm_count CTAs x (planes per chunk + z halo)).  Synchronises the stream.
  * PS_EINVAL: fused kernel not available for this grid, values out of range. */

@@ -362,9 +362,10 @@ int ps_get_kernel(const ps_ctx *c) { return c ? c->variant : PS_EINVAL; }
 int ps_set_tuning(ps_ctx *c, int rows_per_thread, int z_chunks)
 {
     if (!c || !c->fused.ok) return PS_EINVAL;
-    if (rows_per_thread < 0 || rows_per_thread > 1 || z_chunks < 0 || z_chunks > c->g.nz / 2)
+    if (rows_per_thread < 0 || rows_per_thread > 2 || z_chunks < 0 || z_chunks > c->g.nz / 2)
         return PS_EINVAL;
-    const int rpt = 1;
+    const int rpt = rows_per_thread ? rows_per_thread : c->fused.rpt;
+    if (c->variant == PS_KERNEL_FUSED_OTF && rpt != 1) return PS_EINVAL;
     PS_CUDA(cudaStreamSynchronize(c->stream));
     const cudaError_t e = ps::zm_plan_tiles(&c->fused, c->g, rpt, z_chunks);
     if (e == cudaErrorInvalidValue) { cudaGetLastError(); return PS_EINVAL; }

@@ -42,11 +42,12 @@ def assert_p_parity(p_gpu, p_ora, what=""):
     assert nbad == 0, f"{what}: {nbad} doubles differ (max-rel {diff:.3e})"
 
 
-def variants_for(B, w, tunings=((1, 0), (1, 1), (1, 3), (2, 0))):
+def variants_for(B, w, tunings=((1, 0), (1, 1), (1, 3), (2, 0), (2, 2))):
     """Kernel variants the library accepts for this grid shape (asked of the library itself):
     (kernel, rows_per_thread, z_chunks); the fused kernel is run in several launch geometries."""
     out = []
     with B.PoissonSolver(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, workspace=False) as s:
+        # FUSED_OTF before FUSED: it takes one row per thread only and the tunings below end on 2
         for v in (B.KERNEL_TWOPASS, B.KERNEL_RESIDENT, B.KERNEL_FUSED_OTF, B.KERNEL_FUSED):
             try:
                 s.set_kernel(v)
