@@ -310,7 +310,7 @@ def run_ours(args, rank):
         torch.cuda.synchronize()
         to_tol = {"seconds": time.perf_counter() - t0, "cycles": mg.sweeps, "levels": levels,
                   "converged": bool(mg.converged), "res_rel": mg.res_rel,
-                  "method": "multigrid V(2,2) cycles, red-black SOR smoother (binding defaults)",
+                  "method": "multigrid V(0,2) cycles, red-black SOR smoother (binding defaults)",
                   "plain_sor": "see profiles/r01_five_configs.md (config 4: not converged after "
                                "1e6 sweeps / 303 s)"}
 

@@ -258,13 +258,14 @@ class PoissonSolver:
         return ra.value, rr.value, bn.value
 
     # -- multigrid acceleration
-    def mg_setup(self, levels: int = 6, nu1: int = 2, nu2: int = 2, coarse_sweeps: int = 100,
-                 gamma: int = 1, omega_s: float = 1.7, nu_growth: int = 4,
+    def mg_setup(self, levels: int = 6, nu1: int = 0, nu2: int = 2, coarse_sweeps: int = 30,
+                 gamma: int = 1, omega_s: float = 1.75, nu_growth: int = 4,
                  nu_max: int = 16) -> int:
         """Build the level hierarchy from the current coefficients; returns the levels in use.
-        The defaults are the setting measured fastest to 1e-8 on the bubbly ducts
-        (profiles/r01_five_configs.md): V(2,2) on the finest level, 4x more smoothing per
-        coarser level up to 16, 100 sweeps on the coarsest of 6 levels, omega_s = 1.7."""
+        The defaults are the setting measured fastest to 1e-8 on all five configs
+        (profiles/r01_five_configs.md): V(0,2) -- no pre-smoothing, 2 post-smoothing
+        sweeps on the finest level, 4x more per coarser level up to 16 --, 30 sweeps on the
+        coarsest of 6 levels, omega_s = 1.75 (V(0,2) diverges from omega_s = 1.85 on)."""
         self._sync_stream()
         prm = _MgParams(levels, nu1, nu2, nu_growth, nu_max, coarse_sweeps, gamma, omega_s)
         _check(self._lib, self._lib.ps_mg_setup(self._h, ctypes.byref(prm)))

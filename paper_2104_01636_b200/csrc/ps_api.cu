@@ -607,15 +607,46 @@ int mg_nu(int nu, int level, const ps_mg_params &m)
     return (int)(v < m.nu_max ? v : (nu < m.nu_max ? m.nu_max : nu));
 }
 
-// M6: one cycle on the level of context f (level index = depth below the finest).
-int mg_cycle(ps_ctx *f, const ps_mg_params &m, const double *rhs, double *p, int level = 0)
+// The finest level of ps_mg_solve may take its norm inside the residual + restriction pass: with
+// no pre-smoothing there (nu1 = 0) the residual that is restricted is the residual of the
+// iterate the stopping test looks at.  Needs the pair kernel's preconditions.
+bool mg_fused_norm_ok(const ps_ctx *f, const double *rhs, const double *p)
+{
+    return f->child && f->mg_nlev > 1 && mg_nu(f->mgp.nu1, 0, f->mgp) == 0 && f->g.nx % 2 == 0 &&
+           aligned16(rhs, p);
+}
+
+// residual + restriction + norm partials of level f, then the final reduction and the read-back
+int mg_launch_residual_restrict_norm(ps_ctx *f, const double *rhs, const double *p, double *rc,
+                                     double tol)
+{
+    ps::ps_mg_residual_restrict_norm_kernel<<<f->nparts, ps::RED_THREADS, 0, f->stream>>>(
+        f->g, f->ax, f->ay, f->az, rhs, p, rc, f->partR2, f->partB2);
+    f->launches++;
+    PS_CUDA(cudaGetLastError());
+    ps::ps_reduce_final_kernel<<<1, ps::FIN_THREADS, 0, f->stream>>>(f->partR2, f->partB2,
+                                                                    f->nparts, tol, f->scal,
+                                                                    nullptr);
+    f->launches++;
+    PS_CUDA(cudaGetLastError());
+    PS_CUDA(cudaMemcpyAsync(f->h_scal, f->scal, 3 * sizeof(double), cudaMemcpyDeviceToHost,
+                            f->stream));
+    return PS_OK;
+}
+
+// M6: one cycle on the level of context f (level index = depth below the finest).  restricted:
+// the right-hand side of the next level has already been written (fused norm path, level 0).
+int mg_cycle(ps_ctx *f, const ps_mg_params &m, const double *rhs, double *p, int level = 0,
+             bool restricted = false)
 {
     int rc;
     if (!f->child || f->mg_nlev <= 1)
         return run_sweeps(f, rhs, p, m.omega_s, m.coarse_sweeps);
     ps_ctx *k = f->child;
-    if ((rc = run_sweeps(f, rhs, p, m.omega_s, mg_nu(m.nu1, level, m)))) return rc;
-    if ((rc = mg_launch_residual_restrict(f, rhs, p, k->lv_rhs))) return rc;
+    if (!restricted) {
+        if ((rc = run_sweeps(f, rhs, p, m.omega_s, mg_nu(m.nu1, level, m)))) return rc;
+        if ((rc = mg_launch_residual_restrict(f, rhs, p, k->lv_rhs))) return rc;
+    }
     PS_CUDA(cudaMemsetAsync(k->lv_p, 0, k->g.cells() * sizeof(double), f->stream));
     for (int g = 0; g < m.gamma; ++g)
         if ((rc = mg_cycle(k, m, k->lv_rhs, k->lv_p, level + 1))) return rc;
@@ -679,6 +710,29 @@ int ps_mg_solve(ps_ctx *c, const double *rhs_dev, double *p_dev, int max_cycles,
     if (!c->have_coef || !c->mg_ready) return PS_ESTATE;
     for (ps_ctx *k = c->child; k; k = k->child) k->stream = c->stream;
     int cyc = 0, converged = 0, rc = 0;
+    if (mg_fused_norm_ok(c, rhs_dev, p_dev) && max_cycles > 0) {
+        // (cycle, check)* as below, but the check of cycle n rides on the residual + restriction
+        // pass that opens cycle n + 1 (one pass of 41 B/cell instead of 40 + 41); the pass after
+        // the last cycle only serves the norm
+        for (cyc = 0;; ++cyc) {
+            if ((rc = mg_launch_residual_restrict_norm(c, rhs_dev, p_dev, c->child->lv_rhs, tol)))
+                return rc;
+            if (cyc >= 1) {
+                PS_CUDA(cudaStreamSynchronize(c->stream));
+                if (tol > 0.0 && c->h_scal[1] <= tol) { converged = 1; break; }
+                if (cyc == max_cycles) break;
+            }
+            if ((rc = mg_cycle(c, c->mgp, rhs_dev, p_dev, 0, true))) return rc;
+        }
+        if (info) {
+            info->sweeps = cyc;
+            info->converged = converged;
+            info->res_abs = c->h_scal[0];
+            info->res_rel = c->h_scal[1];
+            info->rhs_norm = c->h_scal[2];
+        }
+        return PS_OK;
+    }
     for (cyc = 1; cyc <= max_cycles; ++cyc) {
         if ((rc = mg_cycle(c, c->mgp, rhs_dev, p_dev))) return rc;
         if ((rc = enqueue_residual(c, rhs_dev, p_dev, tol))) return rc;

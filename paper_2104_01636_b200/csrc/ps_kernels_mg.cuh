@@ -91,6 +91,57 @@ ps_mg_residual_restrict_pair_kernel(Grid gf, const double *__restrict__ ax,
     }
 }
 
+// M2 + M3 + the norms of row a4 in one pass (used by ps_mg_solve when the finest level has no
+// pre-smoothing: the residual the restriction needs is then the residual of the iterate whose
+// norm decides the stop, so the separate 40 B/cell norm pass of every cycle is saved).
+// Block b owns the coarse cells [512 b, 512 b + 512) = RED_CHUNK fine cells; thread t takes
+// coarse cells t and t + 256 of them and adds r^2 (and rhs^2) of its 16 children in the order
+// (x, y, z fastest to slowest), then the fixed block tree: the partials depend on N only, like
+// those of ps_residual_partial_kernel (a different, equally fixed tree: the two norms agree to
+// rounding, not bitwise).
+__global__ void __launch_bounds__(RED_THREADS)
+ps_mg_residual_restrict_norm_kernel(Grid gf, const double *__restrict__ ax,
+                                    const double *__restrict__ ay, const double *__restrict__ az,
+                                    const double *__restrict__ rhs, const double *__restrict__ p,
+                                    double *__restrict__ rc, double *__restrict__ partR2,
+                                    double *__restrict__ partB2)
+{
+    __shared__ double sm[RED_THREADS / 32];
+    const int cx = gf.nx >> 1, cy = gf.ny >> 1, cz = gf.nz >> 1;
+    const size_t NC = (size_t)cx * cy * cz;
+    const size_t base = (size_t)blockIdx.x * (RED_CHUNK / 8);
+    double r2 = 0.0, b2 = 0.0;
+#pragma unroll 1
+    for (int m = 0; m < RED_CHUNK / 8 / RED_THREADS; ++m) {
+        const size_t c = base + (size_t)m * RED_THREADS + threadIdx.x;
+        if (c < NC) {
+            const int I = (int)((unsigned)c % (unsigned)cx);
+            const unsigned t = (unsigned)c / (unsigned)cx;
+            const int J = (int)(t % (unsigned)cy), K = (int)(t / (unsigned)cy);
+            double acc = 0.0;
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const int i = 2 * I, j = 2 * J + (q & 1), k = 2 * K + (q >> 1);
+                double2 b;
+                const double2 r = residual_pair(gf, ax, ay, az, rhs, p, i, j, k, gf.idx(i, j, k), b);
+                acc = (q == 0) ? r.x : acc + r.x;
+                acc = acc + r.y;
+                r2 = r2 + r.x * r.x;
+                r2 = r2 + r.y * r.y;
+                b2 = b2 + b.x * b.x;
+                b2 = b2 + b.y * b.y;
+            }
+            rc[c] = 0.125 * acc;
+        }
+    }
+    const double Rs = block_tree_sum<RED_THREADS>(r2, sm);
+    const double Bs = block_tree_sum<RED_THREADS>(b2, sm);
+    if (threadIdx.x == 0) {
+        partR2[blockIdx.x] = Rs;
+        partB2[blockIdx.x] = Bs;
+    }
+}
+
 // M2 alone (kept for tests of the residual field).
 __global__ void __launch_bounds__(256)
 ps_mg_residual_field_kernel(Grid g, const double *__restrict__ ax, const double *__restrict__ ay,

@@ -90,6 +90,7 @@ PARAMS = [
     dict(levels=3, nu1=2, nu2=2, coarse_sweeps=30, gamma=2, omega_s=1.3, nu_growth=1, nu_max=64),
     dict(levels=1, nu1=0, nu2=0, coarse_sweeps=5, gamma=1, omega_s=1.5, nu_growth=1, nu_max=64),     # plain SOR
     dict(levels=99, nu1=2, nu2=1, coarse_sweeps=40, gamma=1, omega_s=1.6, nu_growth=4, nu_max=16),
+    dict(levels=99, nu1=0, nu2=2, coarse_sweeps=30, gamma=1, omega_s=1.75, nu_growth=4, nu_max=16),  # the binding defaults
 ]
 
 
@@ -128,6 +129,47 @@ def test_config1_to_tolerance_same_cycle_count(torch_cuda, B, ora):
     assert abs(ig.res_rel - io.res_rel) <= NORM_TOL * io.res_rel
     # the answer is the solution of the linear system: the oracle's own O5 norm on the GPU's p
     assert ora.residual(coef, w.rhs, p_d.cpu().numpy())[1] <= 1e-8
+
+
+def test_fused_norm_path_defaults_to_tolerance(torch_cuda, B, ora):
+    """With no pre-smoothing on the finest level (the binding defaults, V(0,2)) ps_mg_solve takes
+    the norm of every cycle inside the residual + restriction pass of the next one.  The
+    (cycle, check)* semantics must not change: same cycle count as the oracle's plain loop, p
+    bitwise, norms to 1e-10 (a different fixed summation tree), at least one cycle even from a
+    converged start, max_cycles honoured, max_cycles = 0 only measures."""
+    w = wl.make_config(1)
+    prm = dict(levels=6, nu1=0, nu2=2, coarse_sweeps=30, gamma=1, omega_s=1.75, nu_growth=4, nu_max=16)
+    coef = ora.coefficients(w.F, w.rho_l, w.rho_g, w.dx, w.dy, w.dz)
+    p_o = np.zeros_like(w.rhs)
+    io = ora.mg_solve(coef, w.rhs, p_o, 200, 1e-8, **prm)
+    assert io.converged
+    with B.PoissonSolver(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz) as s:
+        s.set_fraction(dev(torch_cuda, w.F), w.rho_l, w.rho_g)
+        s.mg_setup()                                             # the defaults are prm
+        rhs_d = dev(torch_cuda, w.rhs)
+        p_d = torch_cuda.zeros(w.rhs.shape, dtype=torch_cuda.float64, device="cuda")
+        ig = s.mg_solve(rhs_d, p_d, 200, 1e-8)
+        assert ig.converged and ig.sweeps == io.sweeps
+        same(p_d.cpu().numpy(), p_o, "config 1, default multigrid")
+        assert abs(ig.res_rel - io.res_rel) <= NORM_TOL * io.res_rel
+        ra, rr, bn = s.residual(rhs_d, p_d)                      # the a4 kernel on the same p
+        assert abs(ig.res_rel - rr) <= NORM_TOL * rr and abs(ig.rhs_norm - bn) <= NORM_TOL * bn
+        # converged start: still one cycle, as in the oracle's loop
+        q_o = p_o.copy()
+        jo = ora.mg_solve(coef, w.rhs, q_o, 200, 1e-8, **prm)
+        jg = s.mg_solve(rhs_d, p_d, 200, 1e-8)
+        assert (jg.sweeps, jg.converged) == (jo.sweeps, jo.converged) == (1, 1)
+        same(p_d.cpu().numpy(), q_o, "one more cycle from the converged iterate")
+        # max_cycles reached without convergence; max_cycles = 0 leaves p alone
+        p_d.zero_()
+        p3 = np.zeros_like(w.rhs)
+        ko = ora.mg_solve(coef, w.rhs, p3, 3, 1e-8, **prm)
+        kg = s.mg_solve(rhs_d, p_d, 3, 1e-8)
+        assert (kg.sweeps, kg.converged) == (ko.sweeps, ko.converged) == (3, 0)
+        same(p_d.cpu().numpy(), p3, "three default cycles")
+        zg = s.mg_solve(rhs_d, p_d, 0, 1e-8)
+        assert zg.sweeps == 0 and abs(zg.res_rel - kg.res_rel) <= NORM_TOL * kg.res_rel
+        same(p_d.cpu().numpy(), p3, "max_cycles = 0")
 
 
 def test_config3_three_cycles_and_state_errors(torch_cuda, B, ora):
