@@ -433,3 +433,31 @@ def test_wide_dynamic_range_bitwise(torch_cuda, B, ora):
                 s.sweeps(to_dev(torch_cuda, rhs), p_d, w.omega, nsweeps)
                 p_gpu = p_d.cpu().numpy()
                 assert int(np.count_nonzero(p_gpu != p_ora)) == 0, f"variant {variant} x{nsweeps}"
+
+
+def test_subnormal_coefficients_bitwise(torch_cuda, B, ora):
+    """Densities near the top of the fp64 range with h = 1 give SUBNORMAL face coefficients
+    (2 / 1.6e308): the coefficient quotients of the on-the-fly variant leave the fast path of the
+    division (its guards ask for a normal quotient) and must fall back to the plain quotient; the
+    stored-coefficient kernels get the same subnormals from ps_set_fraction.  All equal the
+    oracle bit for bit."""
+    nx, ny, nz = 40, 20, 8
+    w = wl.make_custom(nx, ny, nz, 0, 0, 3, dx=1.0, dy=1.0, dz=1.0)
+    w.F = wl.random_fraction(nx, ny, nz, 3)
+    rho_l, rho_g = 8.0e307, 4.0e307
+    coef = ora.coefficients(w.F, rho_l, rho_g, 1.0, 1.0, 1.0)
+    sub = (coef[2] > 0.0) & (coef[2] < 2.2e-308)
+    assert coef[2].min() > 0.0 and sub.mean() > 0.5                # most az are subnormal
+    p_ora = np.zeros_like(w.rhs)
+    ora.sweep(coef, w.rhs, p_ora, w.omega, 2)
+    assert np.isfinite(p_ora).all()
+    for kernel in (B.KERNEL_TWOPASS, B.KERNEL_FUSED, B.KERNEL_FUSED_OTF):
+        with B.PoissonSolver(nx, ny, nz, 1.0, 1.0, 1.0) as s:
+            s.set_kernel(kernel)
+            s.set_fraction(to_dev(torch_cuda, w.F), rho_l, rho_g)
+            if kernel == B.KERNEL_FUSED:
+                gz = s.export_coefficients()[2].cpu().numpy()
+                assert np.array_equal(gz, coef[2])
+            p_d = torch_cuda.zeros(nz, ny, nx, dtype=torch_cuda.float64, device="cuda")
+            s.sweeps(to_dev(torch_cuda, w.rhs), p_d, w.omega, 2)
+            assert int(np.count_nonzero(p_d.cpu().numpy() != p_ora)) == 0, f"kernel {kernel}"
