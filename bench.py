@@ -301,6 +301,11 @@ def run_ours(args, rank):
     # accelerated solve, outside the throughput window, wall clock incl. set-up
     to_tol = None
     if not args.no_mg:
+        # warm-up, untimed: allocates the level hierarchy and loads the multigrid kernels once (as
+        # a time stepper would have after its first step); the timed solve below still pays the
+        # coefficient build, the coarsening of all levels and every cycle
+        s.mg_setup()
+        s.mg_solve(rhs_d, p_d, 2, 0.0)
         p_d.zero_()
         torch.cuda.synchronize()
         t0 = time.perf_counter()
@@ -310,7 +315,9 @@ def run_ours(args, rank):
         torch.cuda.synchronize()
         to_tol = {"seconds": time.perf_counter() - t0, "cycles": mg.sweeps, "levels": levels,
                   "converged": bool(mg.converged), "res_rel": mg.res_rel,
-                  "method": "multigrid V(0,2) cycles, red-black SOR smoother (binding defaults)",
+                  "method": "multigrid V(0,2) cycles, red-black SOR smoother (binding defaults); "
+                            "timed: ps_set_fraction + ps_mg_setup + ps_mg_solve from p = 0, after "
+                            "an untimed 2-cycle warm-up",
                   "plain_sor": "see profiles/r01_five_configs.md (config 4: not converged after "
                                "1e6 sweeps / 303 s)"}
 
