@@ -461,3 +461,25 @@ def test_subnormal_coefficients_bitwise(torch_cuda, B, ora):
             p_d = torch_cuda.zeros(nz, ny, nx, dtype=torch_cuda.float64, device="cuda")
             s.sweeps(to_dev(torch_cuda, w.rhs), p_d, w.omega, 2)
             assert int(np.count_nonzero(p_d.cpu().numpy() != p_ora)) == 0, f"kernel {kernel}"
+
+
+def test_long_run_repeatable_across_fused_variants(torch_cuda, B):
+    """2,000 sweeps on config 3 (27 tiles x 5 z chunks, every SM busy): the fused kernel twice, its
+    two-rows-per-thread geometry, another z chunking and the on-the-fly variant all end on the same
+    bits -- a rare miss in the mbarrier protocol (a stage read before it landed, a red value read
+    before it was written) would show up as a difference between runs."""
+    w = wl.make_config(3)
+    F_d, rhs_d = to_dev(torch_cuda, w.F), to_dev(torch_cuda, w.rhs)
+    ref = None
+    for kernel, rpt, chunks in [(B.KERNEL_FUSED, 1, 0), (B.KERNEL_FUSED, 1, 0), (B.KERNEL_FUSED, 2, 0),
+                                (B.KERNEL_FUSED, 1, 9), (B.KERNEL_FUSED_OTF, 1, 0)]:
+        with B.PoissonSolver(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz) as s:
+            s.set_kernel(kernel)
+            s.set_tuning(rpt, chunks)
+            s.set_fraction(F_d, w.rho_l, w.rho_g)
+            p_d = torch_cuda.zeros_like(rhs_d)
+            s.sweeps(rhs_d, p_d, w.omega, 2000)
+            if ref is None:
+                ref = p_d.clone()
+            else:
+                assert torch_cuda.equal(p_d, ref), (kernel, rpt, chunks)
