@@ -187,7 +187,11 @@ int ps_mg_levels(const ps_ctx *c);           /* levels in use (0 before ps_mg_se
 
 /* Multigrid cycles c = 1..max_cycles from the caller's p (in/out); after every cycle the
  * deterministic norm of ps_residual; stops at the first cycle with ||r||_2/||rhs||_2 <= tol
- * (tol <= 0: exactly max_cycles cycles).  info->sweeps returns the number of cycles.
+ * (tol <= 0: exactly max_cycles cycles).  info->sweeps returns the number of cycles.  When the
+ * finest level has no pre-smoothing (nu1 = 0) the norm of a cycle is taken inside the residual +
+ * restriction pass that opens the next one (same cycles, same p; the norm agrees with ps_residual
+ * to rounding).  A cycle whose norm is not finite (a diverging parameter set, e.g. V(0,2) with
+ * omega_s >= 1.85) ends the loop with converged = 0.
  * Synchronises the stream once per cycle (the norm read-back).  PS_ESTATE without ps_mg_setup. */
 int ps_mg_solve(ps_ctx *c, const double *rhs_dev, double *p_dev, int max_cycles, double tol,
                 ps_info *info);

@@ -720,7 +720,7 @@ int ps_mg_solve(ps_ctx *c, const double *rhs_dev, double *p_dev, int max_cycles,
             if (cyc >= 1) {
                 PS_CUDA(cudaStreamSynchronize(c->stream));
                 if (tol > 0.0 && c->h_scal[1] <= tol) { converged = 1; break; }
-                if (cyc == max_cycles) break;
+                if (cyc == max_cycles || !std::isfinite(c->h_scal[1])) break;
             }
             if ((rc = mg_cycle(c, c->mgp, rhs_dev, p_dev, 0, true))) return rc;
         }
@@ -738,6 +738,7 @@ int ps_mg_solve(ps_ctx *c, const double *rhs_dev, double *p_dev, int max_cycles,
         if ((rc = enqueue_residual(c, rhs_dev, p_dev, tol))) return rc;
         PS_CUDA(cudaStreamSynchronize(c->stream));
         if (tol > 0.0 && c->h_scal[1] <= tol) { converged = 1; break; }
+        if (!std::isfinite(c->h_scal[1])) break;
     }
     if (cyc > max_cycles) cyc = max_cycles;
     if (max_cycles == 0) {

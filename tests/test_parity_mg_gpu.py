@@ -195,3 +195,16 @@ def test_config3_three_cycles_and_state_errors(torch_cuda, B, ora):
         s.set_fraction(dev(torch_cuda, w.F), w.rho_l, w.rho_g)     # invalidates the hierarchy
         with pytest.raises(B.PsError):
             s.mg_solve(rhs_d, p_d, 1, 0.0)
+
+
+def test_diverging_parameters_stop_early(torch_cuda, B):
+    """V(0,2) with omega_s = 1.9 diverges; ps_mg_solve must not grind through
+    max_cycles on infinities: it stops at the first cycle whose norm is not finite."""
+    w = wl.make_config(1)
+    with B.PoissonSolver(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz) as s:
+        s.set_fraction(dev(torch_cuda, w.F), w.rho_l, w.rho_g)
+        s.mg_setup(omega_s=1.9)
+        p_d = torch_cuda.zeros(w.rhs.shape, dtype=torch_cuda.float64, device="cuda")
+        info = s.mg_solve(dev(torch_cuda, w.rhs), p_d, 100000, 1e-8)
+        assert not info.converged and info.sweeps < 100000
+        assert not np.isfinite(info.res_rel)
