@@ -38,12 +38,21 @@ if ROOT not in sys.path:
 
 METRIC = "poisson_sor_gcell_updates_per_s"
 UNIT = "Gcell-updates/s"
-# algorithmic bytes per cell per sweep-kernel launch:
-#   twopass: one colour per launch, M1 = 40 B/cell/launch (80 B per cell-update)
-#   fused:   one sweep per launch,  M2 = 48 B/cell/launch (48 B per cell-update)
+# algorithmic bytes per cell-update = per cell per SWEEP:
+#   twopass: two launches per sweep, M1 = 40 B/cell/launch = 80 B per cell-update
+#   fused:   one launch per sweep,   M2 = 48 B per cell-update
 #   fused_otf: the same with rho (8 B) in place of ax, ay, az (24 B) = 32 B per cell-update
-ALGO_BYTES_PER_CELL_LAUNCH = {"twopass": 40.0, "fused": 48.0, "fused_otf": 32.0,
-                              "resident": 80.0}   # resident: L2-resident grids only, per sweep
+#   resident: many sweeps per cooperative launch on an L2-resident grid; 80 B per cell-update of
+#             L2 (not HBM) traffic -- reported, but not an HBM roofline
+ALGO_BYTES_PER_UPDATE = {"twopass": 80.0, "fused": 48.0, "fused_otf": 32.0, "resident": 80.0}
+
+
+# Plain red-black SOR (row a5 alone) on the configs where a live run to 1e-8 does not fit a bench:
+# measured once on one B200 with `python -m paper_2104_01636_b200.report` (profiles/).
+PLAIN_SOR_RECORDED = {
+    4: {"converged": False, "sweeps": 1_000_000, "seconds": 302.9, "res_rel": 2.458e-06,
+        "source": "profiles/r01_five_configs.md (round 1, ps_solve, omega 1.6, K = 50)"},
+}
 
 
 def parse_args():
@@ -56,7 +65,10 @@ def parse_args():
     ap.add_argument("--sweeps", type=int, default=0, help="sweeps per step (default: the config's)")
     ap.add_argument("--kernel", default="auto",
                     choices=["auto", "twopass", "fused", "resident", "fused_otf"])
-    ap.add_argument("--no-mg", action="store_true", help="skip the multigrid time-to-1e-8 leg")
+    ap.add_argument("--no-mg", action="store_true", help="skip the time-to-1e-8 legs")
+    ap.add_argument("--sor-sweeps", type=int, default=-1,
+                    help="cap of the live plain-SOR solve to 1e-8 (default: 1e6 for grids up to "
+                         "8M cells, 20000 beyond; 0 = skip)")
     ap.add_argument("--rpt", type=int, default=0, help="fused kernel: rows per thread (0 = auto)")
     ap.add_argument("--zchunks", type=int, default=0, help="fused kernel: z chunks (0 = auto)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -135,12 +147,25 @@ def measured_peak():
 
 
 def ncu_traffic(kernel: str, cfg: int):
-    """DRAM bytes per launch of the sweep kernel from the committed ncu summary, or None."""
+    """(DRAM bytes per launch of the sweep kernel from the committed `ncu --set full` summary,
+    where it comes from) or (None, why).  profiles/traffic.json records the sha256 of the kernel
+    source the capture was taken with; a capture of another kernel version is stale and is NOT
+    reported."""
+    import hashlib
     try:
         with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
-            return json.load(f).get(f"{kernel}:config{cfg}")
+            rec = json.load(f)
+        with open(os.path.join(ROOT, "paper_2104_01636_b200", "csrc", "ps_kernels_zmarch.cuh"), "rb") as f:
+            sha = hashlib.sha256(f.read()).hexdigest()[:16]
     except (OSError, ValueError):
-        return None
+        return None, "profiles/traffic.json missing"
+    val = rec.get(f"{kernel}:config{cfg}")
+    if val is None:
+        return None, "no ncu capture of this kernel/config"
+    if rec.get("kernel_source_sha16") != sha:
+        return None, (f"stale: capture of kernel source {rec.get('kernel_source_sha16')}, "
+                      f"current {sha}")
+    return val, rec.get("_source")
 
 
 # --------------------------------------------------------------------------- oracle legs
@@ -268,7 +293,7 @@ def run_ours(args, rank):
     replicas.barrier(rank)
     launches = s.launch_count() - l0
     secs = ev0.elapsed_time(ev1) / 1e3
-    sweep_ms, sweep_launches = s.timing()
+    sweep_ms, sweep_launches, sweeps_timed = s.timing()
     s.enable_timing(False)
     clk = clocks.stop() if rank.rank == 0 else None
     value, units, tmax = replicas.aggregate_throughput(rank, float(w.cells) * sweeps * args.steps,
@@ -314,19 +339,43 @@ def run_ours(args, rank):
         mg = s.mg_solve(rhs_d, p_d, 1000, 1e-8)
         torch.cuda.synchronize()
         to_tol = {"seconds": time.perf_counter() - t0, "cycles": mg.sweeps, "levels": levels,
-                  "converged": bool(mg.converged), "res_rel": mg.res_rel,
-                  "method": "multigrid V(0,2) cycles, red-black SOR smoother (binding defaults); "
-                            "timed: ps_set_fraction + ps_mg_setup + ps_mg_solve from p = 0, after "
-                            "an untimed 2-cycle warm-up",
-                  "plain_sor": "see profiles/r01_five_configs.md (config 4: not converged after "
-                               "1e6 sweeps / 303 s)"}
+                  "converged": bool(mg.converged), "res_rel": mg.res_rel, "solver": "multigrid",
+                  "method": "multigrid cycles around the red-black SOR smoother (PAPER.md:78; "
+                            "binding defaults, DESIGN.md §12); timed: ps_set_fraction + "
+                            "ps_mg_setup + ps_mg_solve from p = 0, after an untimed 2-cycle "
+                            "warm-up"}
+        if rank.rank == 0 and not args.no_cpu_baseline:
+            # the oracle's own O5 norm of the GPU's final p (outside every timed region): the
+            # headline time carries its oracle check
+            import oracle
+            oracle.build()
+            coef = oracle.coefficients(w.F, w.rho_l, w.rho_g, w.dx, w.dy, w.dz)
+            to_tol["oracle_res_rel"] = oracle.residual(coef, w.rhs, p_d.cpu().numpy())[1]
+            del coef
+        # the row-(a5) loop on its own (plain red-black SOR at the config's omega, no multigrid):
+        # live up to --sor-sweeps sweeps; beyond that the round's recorded long run is quoted
+        sor_cap = args.sor_sweeps if args.sor_sweeps >= 0 else (1_000_000 if w.cells <= 8e6 else 20_000)
+        if sor_cap > 0:
+            p_d.zero_()
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            si = s.solve(rhs_d, p_d, w.omega, sor_cap, 1e-8)
+            torch.cuda.synchronize()
+            to_tol["plain_sor"] = {"converged": bool(si.converged), "sweeps": si.sweeps,
+                                   "seconds": time.perf_counter() - t0, "res_rel": si.res_rel,
+                                   "omega": w.omega, "live": True, "max_sweeps": sor_cap}
+            rec = PLAIN_SOR_RECORDED.get(args.config)
+            if rec and not si.converged:
+                to_tol["plain_sor"]["recorded_long_run"] = rec
 
     if rank.rank != 0:
         return
     peak, peak_src = measured_peak()
     launch_s = sweep_ms / 1e3 / max(sweep_launches, 1)
-    algo_bytes = ALGO_BYTES_PER_CELL_LAUNCH[kname] * w.cells
-    achieved = algo_bytes / launch_s / 1e9
+    sweep_s = sweep_ms / 1e3 / max(sweeps_timed, 1)
+    algo_bytes = ALGO_BYTES_PER_UPDATE[kname] * w.cells            # per sweep
+    achieved = algo_bytes / sweep_s / 1e9
+    traffic, traffic_src = ncu_traffic(kname, args.config)
     line = {
         "metric": METRIC, "value": value / 1e9, "unit": UNIT, "n_gpus": rank.world,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tmax / args.steps,
@@ -339,14 +388,18 @@ def run_ours(args, rank):
                          else "L2-resident working set (not an HBM measurement)",
                    "parallelism": "replicas" if rank.world > 1 else "single GPU"},
         "final_res_rel": info.res_rel,
-        "sweep_only_gcells_per_s": w.cells * (sweep_launches * (0.5 if kname == "twopass" else 1.0))
-                                   / (sweep_ms / 1e3) / 1e9 if sweep_ms > 0 else None,
+        "sweep_only_gcells_per_s": w.cells * sweeps_timed / (sweep_ms / 1e3) / 1e9
+                                   if sweep_ms > 0 else None,
         "gpu_launches": launches,
         "clocks": clk,
-        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                     "frac": achieved / peak, "traffic": ncu_traffic(kname, args.config),
-                     "kernel": kname, "algorithmic_bytes_per_launch": algo_bytes,
-                     "avg_launch_ms": 1e3 * launch_s, "launches_timed": sweep_launches,
+        "roofline": {"bound": "hbm" if kname != "resident" else "l2 (grid is L2-resident: not an "
+                                                                  "HBM measurement)",
+                     "achieved": achieved, "peak": peak, "unit": "GB/s",
+                     "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_src,
+                     "kernel": kname, "algorithmic_bytes_per_sweep": algo_bytes,
+                     "launches_per_sweep": sweep_launches / max(sweeps_timed, 1),
+                     "avg_sweep_ms": 1e3 * sweep_s, "avg_launch_ms": 1e3 * launch_s,
+                     "launches_timed": sweep_launches, "sweeps_timed": sweeps_timed,
                      "peak_source": peak_src},
     }
     if e2e:

@@ -23,7 +23,10 @@
  *
  * Pointers
  *   *_dev  : device memory owned by the caller (e.g. a torch tensor), contiguous natural layout,
- *            16-byte aligned, nx*ny*nz doubles.  Never freed or retained past the call.
+ *            16-byte aligned, nx*ny*nz doubles.  Never freed or retained past the call.  A field
+ *            pointer that is not 16-byte aligned is rejected with PS_EINVAL by every entry point
+ *            (the kernels use 16-byte accesses and TMA; which kernel runs, and hence the
+ *            summation tree of the norms, depends on the grid shape only, never on an address).
  *   *_host : host memory owned by the caller (pageable or pinned), same layout.
  *   Output scalars / ps_info are host pointers.
  *
@@ -68,7 +71,9 @@ typedef struct {
     double rhs_norm;    /* || rhs ||_2                                                     */
 } ps_info;
 
-/* Create a solver for an nx x ny x nz grid with spacings dx,dy,dz on the current CUDA device.
+/* Create a solver for the paper's problem statement: a uniform Cartesian collocated grid
+ * (PAPER.md:45 §2, :199 §4) of nx x ny x nz cells with spacings dx,dy,dz, duct walls in x and y
+ * and periodic z (§4), on the current CUDA device.
  * PS_EINVAL: out NULL; nx,ny < 1; nz < 2 or nz odd (the red-black colouring must stay
  * consistent across the periodic wrap); dx,dy,dz not finite or <= 0.
  * Allocates its own workspace (ps_workspace_bytes) with cudaMalloc unless ps_set_workspace
@@ -118,7 +123,10 @@ int ps_set_fraction(ps_ctx *c, const double *F_dev, double rho_l, double rho_g);
 /* Copy the face coefficients out in natural layout (device pointers, any may be NULL). */
 int ps_export_coefficients(ps_ctx *c, double *ax_dev, double *ay_dev, double *az_dev);
 
-/* Red-black SOR on A p = rhs starting from the caller's p (in/out).
+/* Step 11 of the paper's time step, div(grad p / rho) = rhs (§2.2), by the
+ * "red black SOR relaxation scheme" of PAPER.md:78 §2.1: red-black SOR on A p = rhs starting from
+ * the caller's p (in/out).  omega, colour order, norm and stopping rule are readings S3-S5 of
+ * DESIGN.md §2 (the paper gives none).
  *   for s = 1..max_sweeps { red; black; if (tol > 0 && (s % K == 0 || s == max_sweeps)) check }
  * stopping at the first check with ||r||_2/||rhs||_2 <= tol.  tol <= 0: exactly max_sweeps
  * sweeps, norm computed once at the end.  Synchronises the stream before returning; the only
@@ -136,15 +144,20 @@ int ps_sweeps(ps_ctx *c, const double *rhs_dev, double *p_dev, double omega, int
  * asynchronous.  For parity tests of the half-sweep itself. */
 int ps_half_sweep(ps_ctx *c, const double *rhs_dev, double *p_dev, double omega, int colour);
 
-/* ||rhs - A p||_2 and its ratio to ||rhs||_2 by the deterministic two-pass reduction
+/* Residual of step 11's equation (the norm is reading S5 of DESIGN.md §2, the paper
+ * states none): ||rhs - A p||_2 and its ratio to ||rhs||_2 by the deterministic two-pass reduction
  * (fixed partition, warp-shuffle tree, single-block fixed-order final pass; no atomics).
  * Synchronises the stream.  Outputs are host pointers; res_rel / rhs_norm may be NULL. */
 int ps_residual(ps_ctx *c, const double *rhs_dev, const double *p_dev, double *res_abs,
                 double *res_rel, double *rhs_norm);
 
 /* The whole path on HOST buffers (the end-to-end leg of bench.py): H2D of F and rhs and p,
- * ps_set_fraction, ps_solve, D2H of p.  Staging buffers live in the context and are allocated
- * on first use.  Same errors as the calls it wraps. */
+ * ps_set_fraction, ps_solve, D2H of p.  The three device staging fields come from the caller's
+ * ps_set_host_staging block (256-byte aligned, >= ps_host_staging_bytes, retained until
+ * ps_destroy or replaced) or, without one, from a cudaMalloc on first use.  Same errors as the
+ * calls it wraps. */
+size_t ps_host_staging_bytes(const ps_ctx *c);
+int ps_set_host_staging(ps_ctx *c, void *st_dev, size_t bytes);
 int ps_solve_host(ps_ctx *c, const double *F_host, double rho_l, double rho_g,
                   const double *rhs_host, double *p_host, double omega, int max_sweeps,
                   double tol, ps_info *info);
@@ -153,9 +166,10 @@ int ps_solve_host(ps_ctx *c, const double *F_host, double rho_l, double rho_g,
  * every batch of sweep launches issued by ps_solve / ps_sweeps / ps_solve_host is bracketed by a
  * pair of CUDA events on the context's stream.  ps_timing synchronises the stream, adds up the
  * elapsed times since the last ps_timing call and returns them with the number of sweep-kernel
- * launches they cover (sweep_ms / launches = average launch duration); either may be NULL. */
+ * launches and the number of sweeps they cover (the resident kernel runs many sweeps per launch,
+ * the two-pass kernel half a sweep); any output may be NULL. */
 int ps_enable_timing(ps_ctx *c, int on);
-int ps_timing(ps_ctx *c, double *sweep_ms, long long *sweep_launches);
+int ps_timing(ps_ctx *c, double *sweep_ms, long long *sweep_launches, long long *sweeps);
 
 /* ------------------------------------------------------------------------------------------
  * Multigrid acceleration of the red-black SOR ("multigrid accelerated red black SOR
@@ -178,10 +192,21 @@ typedef struct {
     double omega_s;      /* relaxation factor of smoother and coarsest solver, in (0,2)        */
 } ps_mg_params;
 
+/* Device memory of the coarse levels (per level: coefficients, ping-pong buffer, reduction
+ * partials, right-hand side, correction).  ps_mg_workspace_bytes: bytes a hierarchy of `levels`
+ * levels (clipped like ps_mg_setup clips them) needs.  ps_mg_set_workspace hands the context a
+ * caller-owned block (256-byte aligned; retained until ps_destroy or replaced; any existing
+ * hierarchy is dropped).  Without one the library allocates the block itself with cudaMalloc at
+ * the first ps_mg_setup and frees it in ps_destroy. */
+size_t ps_mg_workspace_bytes(const ps_ctx *c, int levels);
+int ps_mg_set_workspace(ps_ctx *c, void *ws_dev, size_t bytes);
+
 /* Build the level hierarchy from the coefficients of the last ps_set_fraction (one coarsening
- * launch per level; device memory for the levels is allocated by the library and freed by
- * ps_destroy or the next ps_mg_setup).  Must be called again after every ps_set_fraction.
- * PS_EINVAL: bad parameters.  PS_ESTATE: no coefficients. */
+ * launch per level).  Must be called again after every ps_set_fraction; the level contexts and
+ * their memory are reused as long as the depth does not change.  On any failure the hierarchy is
+ * dropped (ps_mg_levels() == 0) and ps_mg_solve returns PS_ESTATE until a set-up succeeds.
+ * PS_EINVAL: bad parameters; a caller-owned level block that is too small; the current CUDA
+ * device is not the one the context was created on.  PS_ESTATE: no coefficients. */
 int ps_mg_setup(ps_ctx *c, const ps_mg_params *prm);
 int ps_mg_levels(const ps_ctx *c);           /* levels in use (0 before ps_mg_setup) */
 

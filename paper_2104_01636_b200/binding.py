@@ -25,8 +25,8 @@ SYMBOLS = ("ps_create", "ps_destroy", "ps_workspace_bytes", "ps_set_workspace", 
            "ps_set_check_interval", "ps_set_kernel", "ps_get_kernel", "ps_set_tuning",
            "ps_get_tuning", "ps_set_fraction",
            "ps_export_coefficients", "ps_solve", "ps_sweeps", "ps_half_sweep", "ps_residual",
-           "ps_solve_host", "ps_enable_timing", "ps_timing", "ps_launch_count", "ps_strerror",
-           "ps_mg_setup", "ps_mg_levels", "ps_mg_solve", "ps_mg_export_coarse",
+           "ps_solve_host", "ps_host_staging_bytes", "ps_set_host_staging", "ps_enable_timing", "ps_timing", "ps_launch_count", "ps_strerror",
+           "ps_mg_workspace_bytes", "ps_mg_set_workspace", "ps_mg_setup", "ps_mg_levels", "ps_mg_solve", "ps_mg_export_coarse",
            "ps_mg_residual_restrict", "ps_mg_prolong_add", "ps_rhs_from_velocity",
            "ps_correct_velocity", "ps_face_divergence", "ps_ssf_rhs")
 
@@ -93,7 +93,14 @@ def load(path: str | None = None) -> ctypes.CDLL:
     lib.ps_residual.argtypes = [vp, vp, vp, dp, dp, dp]
     lib.ps_solve_host.argtypes = [vp, vp, d, d, vp, vp, d, i, d, ctypes.POINTER(_Info)]
     lib.ps_enable_timing.argtypes = [vp, i]
-    lib.ps_timing.argtypes = [vp, dp, ctypes.POINTER(ctypes.c_longlong)]
+    lib.ps_host_staging_bytes.argtypes = [vp]
+    lib.ps_host_staging_bytes.restype = ctypes.c_size_t
+    lib.ps_set_host_staging.argtypes = [vp, vp, ctypes.c_size_t]
+    llp = ctypes.POINTER(ctypes.c_longlong)
+    lib.ps_timing.argtypes = [vp, dp, llp, llp]
+    lib.ps_mg_workspace_bytes.argtypes = [vp, i]
+    lib.ps_mg_workspace_bytes.restype = ctypes.c_size_t
+    lib.ps_mg_set_workspace.argtypes = [vp, vp, ctypes.c_size_t]
     lib.ps_launch_count.argtypes = [vp]
     lib.ps_launch_count.restype = ctypes.c_longlong
     lib.ps_mg_setup.argtypes = [vp, ctypes.POINTER(_MgParams)]
@@ -123,6 +130,9 @@ def _dev_ptr(t, shape, name):
     if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64
             and t.is_contiguous() and tuple(t.shape) == tuple(shape)):
         raise TypeError(f"{name}: expected a contiguous CUDA float64 tensor of shape {tuple(shape)}")
+    if t.data_ptr() % 16:
+        raise TypeError(f"{name}: device pointer must be 16-byte aligned (a view with an odd "
+                        "storage offset is not; make it contiguous at an even offset)")
     return ctypes.c_void_p(t.data_ptr())
 
 
@@ -150,19 +160,26 @@ class PoissonSolver:
         self.nx, self.ny, self.nz = nx, ny, nz
         self.shape = (nz, ny, nx)
         _check(self._lib, self._lib.ps_create(ctypes.byref(self._h), nx, ny, nz, dx, dy, dz))
-        self._ws = None
+        self._ws = self._mg_ws = self._st_ws = None
+        self._torch_owns = workspace
         if workspace:      # torch owns the device memory (north_star: "PyTorch ... device memory")
             nbytes = self._lib.ps_workspace_bytes(self._h)
-            self._ws = torch.empty(nbytes + 256, dtype=torch.uint8, device="cuda")
-            base = (self._ws.data_ptr() + 255) // 256 * 256
-            _check(self._lib, self._lib.ps_set_workspace(self._h, ctypes.c_void_p(base), nbytes))
+            self._ws, base = self._block(nbytes)
+            _check(self._lib, self._lib.ps_set_workspace(self._h, base, nbytes))
+
+    @staticmethod
+    def _block(nbytes: int):
+        """A torch-owned device block and its 256-byte aligned base pointer."""
+        import torch
+        t = torch.empty(nbytes + 256, dtype=torch.uint8, device="cuda")
+        return t, ctypes.c_void_p((t.data_ptr() + 255) // 256 * 256)
 
     # -- lifetime
     def close(self):
         if getattr(self, "_h", None) is not None and self._h.value:
             self._lib.ps_destroy(self._h)
             self._h = ctypes.c_void_p()
-        self._ws = None
+        self._ws = self._mg_ws = self._st_ws = None
 
     def __del__(self):
         try:
@@ -208,10 +225,12 @@ class PoissonSolver:
         _check(self._lib, self._lib.ps_enable_timing(self._h, int(on)))
 
     def timing(self):
-        """(sweep_ms, sweep_launches) accumulated since the last call; synchronises the stream."""
-        ms, n = ctypes.c_double(), ctypes.c_longlong()
-        _check(self._lib, self._lib.ps_timing(self._h, ctypes.byref(ms), ctypes.byref(n)))
-        return ms.value, n.value
+        """(sweep_ms, sweep_launches, sweeps) accumulated since the last call; synchronises the
+        stream."""
+        ms, n, sw = ctypes.c_double(), ctypes.c_longlong(), ctypes.c_longlong()
+        _check(self._lib, self._lib.ps_timing(self._h, ctypes.byref(ms), ctypes.byref(n),
+                                              ctypes.byref(sw)))
+        return ms.value, n.value, sw.value
 
     def launch_count(self) -> int:
         return self._lib.ps_launch_count(self._h)
@@ -268,6 +287,11 @@ class PoissonSolver:
         coarsest of 6 levels, omega_s = 1.75 (V(0,2) diverges from omega_s = 1.85 on)."""
         self._sync_stream()
         prm = _MgParams(levels, nu1, nu2, nu_growth, nu_max, coarse_sweeps, gamma, omega_s)
+        if self._torch_owns:               # the level memory is a torch allocation too
+            need = self._lib.ps_mg_workspace_bytes(self._h, levels)
+            if need and (self._mg_ws is None or self._mg_ws[0].numel() < need + 256):
+                self._mg_ws = self._block(need)
+                _check(self._lib, self._lib.ps_mg_set_workspace(self._h, self._mg_ws[1], need))
         _check(self._lib, self._lib.ps_mg_setup(self._h, ctypes.byref(prm)))
         return self._lib.ps_mg_levels(self._h)
 
@@ -348,6 +372,10 @@ class PoissonSolver:
                    tol: float) -> Info:
         """Whole path on HOST arrays (numpy or CPU torch tensors); p is updated in place."""
         self._sync_stream()
+        if self._torch_owns and self._st_ws is None:
+            need = self._lib.ps_host_staging_bytes(self._h)
+            self._st_ws = self._block(need)
+            _check(self._lib, self._lib.ps_set_host_staging(self._h, self._st_ws[1], need))
         info = _Info()
         _check(self._lib, self._lib.ps_solve_host(
             self._h, _host_ptr(F, self.shape, "F"), rho_l, rho_g,

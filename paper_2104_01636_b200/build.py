@@ -24,7 +24,10 @@ HEADERS = sorted(f for f in os.listdir(_CSRC) if f.endswith(".cuh"))
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-std=c++17", "-O3", "--fmad=false", "-lineinfo",
-    "-Xcompiler", "-fPIC", "-shared", "-cudart", "static",
+    "-Xcompiler", "-fPIC", "-shared",
+    # the shared CUDA runtime (libcudart.so.12: torch's copy when torch is imported first, else the
+    # toolkit's through the rpath), so the shipped library carries none of the runtime's own code
+    "-cudart", "shared", "-Xlinker", "-rpath=/usr/local/cuda/lib64",
 ]
 
 

@@ -63,21 +63,28 @@ struct ps_ctx {
     size_t ws_bytes;
     bool ws_owned;
     double *ax, *ay, *az, *p_alt, *rho, *partR2, *partB2, *scal;   // scal: 3 doubles out
-    int *done;
+    unsigned *ctr;         // arrival counter of the resident kernel's grid barrier
     int nparts;
+    int device;            // CUDA device the context (and every level below it) lives on
     double *h_scal;        // pinned, 4 doubles
-    // staging of ps_solve_host
+    // staging of ps_solve_host: 3 fields, caller-owned (ps_set_host_staging) or cudaMalloc
     double *st_F, *st_rhs, *st_p;
+    bool st_owned;
     ps::ZmPlan fused;
     // optional event timing of the sweep launches (ps_enable_timing)
     bool timing;
     std::vector<cudaEvent_t> *ev;      // pairs: start, stop
     size_t ev_used;
-    long long timed_launches;
+    long long timed_launches, timed_sweeps;
     // multigrid: the next coarser level is a context of its own; lv_rhs / lv_p are the right-hand
-    // side and the correction of THIS level when it is a coarse one (owned, cudaMalloc)
+    // side and the correction of THIS level when it is a coarse one.  Level memory (workspace of
+    // every coarse context + lv_rhs + lv_p) is carved from the caller's ps_mg_set_workspace block
+    // (mg_ws) or, without one, from one cudaMalloc owned by the finest context (mg_ws_owned).
     ps_ctx *child;
     double *lv_rhs, *lv_p;
+    void *mg_ws;
+    size_t mg_ws_bytes;
+    bool mg_ws_owned;
     ps_mg_params mgp;
     int mg_nlev;           // levels in use below and including this one (0: no hierarchy)
     bool mg_ready;         // hierarchy matches the current coefficients
@@ -85,12 +92,16 @@ struct ps_ctx {
 
 namespace {
 
-size_t field_bytes(const ps_ctx *c) { return align_up(c->g.cells() * sizeof(double), 256); }
+size_t field_bytes_for(size_t cells) { return align_up(cells * sizeof(double), 256); }
+size_t field_bytes(const ps_ctx *c) { return field_bytes_for(c->g.cells()); }
+int nparts_for(size_t cells) { return (int)((cells + ps::RED_CHUNK - 1) / ps::RED_CHUNK); }
 
-size_t workspace_bytes(const ps_ctx *c)
+size_t workspace_bytes_for(size_t cells)
 {
-    return 5 * field_bytes(c) + 2 * align_up((size_t)c->nparts * sizeof(double), 256) + 256 + 256;
+    return 5 * field_bytes_for(cells) +
+           2 * align_up((size_t)nparts_for(cells) * sizeof(double), 256) + 256 + 256;
 }
+size_t workspace_bytes(const ps_ctx *c) { return workspace_bytes_for(c->g.cells()); }
 
 void carve(ps_ctx *c, void *base)
 {
@@ -104,7 +115,7 @@ void carve(ps_ctx *c, void *base)
     c->partR2 = (double *)q; q += pb;
     c->partB2 = (double *)q; q += pb;
     c->scal = (double *)q; q += 256;
-    c->done = (int *)q;
+    c->ctr = (unsigned *)q;
 }
 
 int ensure_workspace(ps_ctx *c)
@@ -156,14 +167,15 @@ int launch_half_sweep(ps_ctx *c, const double *rhs, double *p, double omega, int
     return PS_OK;
 }
 
-// n sweeps on p (in/out), any variant.  The fused variants ping-pong between p and p_alt and
-// leave the result in p (an odd count ends with one device-to-device copy).
-int run_sweeps_untimed(ps_ctx *c, const double *rhs, double *p, double omega, int n);
+// n sweeps, any variant.  The in-place variants work on *cur.  The fused variants ping-pong
+// between the caller's p and p_alt: *cur is the buffer that holds the iterate on entry and on
+// return (p or c->p_alt); callers copy back to p once, when they are done (settle_p).
+int run_sweeps_untimed(ps_ctx *c, const double *rhs, double *p, double **cur, double omega, int n);
 
-int run_sweeps(ps_ctx *c, const double *rhs, double *p, double omega, int n)
+int run_sweeps(ps_ctx *c, const double *rhs, double *p, double **cur, double omega, int n)
 {
     if (n <= 0) return PS_OK;
-    if (!c->timing) return run_sweeps_untimed(c, rhs, p, omega, n);
+    if (!c->timing) return run_sweeps_untimed(c, rhs, p, cur, omega, n);
     if (c->ev_used + 2 > c->ev->size()) {
         cudaEvent_t a, b;
         PS_CUDA(cudaEventCreate(&a));
@@ -173,20 +185,21 @@ int run_sweeps(ps_ctx *c, const double *rhs, double *p, double omega, int n)
     }
     const long long before = c->launches;
     PS_CUDA(cudaEventRecord((*c->ev)[c->ev_used], c->stream));
-    const int rc = run_sweeps_untimed(c, rhs, p, omega, n);
+    const int rc = run_sweeps_untimed(c, rhs, p, cur, omega, n);
     PS_CUDA(cudaEventRecord((*c->ev)[c->ev_used + 1], c->stream));
     c->ev_used += 2;
     c->timed_launches += c->launches - before;
+    c->timed_sweeps += n;
     return rc;
 }
 
-int run_sweeps_untimed(ps_ctx *c, const double *rhs, double *p, double omega, int n)
+int run_sweeps_untimed(ps_ctx *c, const double *rhs, double *p, double **cur, double omega, int n)
 {
     if (c->variant == PS_KERNEL_TWOPASS) {
         for (int s = 0; s < n; ++s) {
-            int rc = launch_half_sweep(c, rhs, p, omega, 0);
+            int rc = launch_half_sweep(c, rhs, *cur, omega, 0);
             if (rc) return rc;
-            rc = launch_half_sweep(c, rhs, p, omega, 1);
+            rc = launch_half_sweep(c, rhs, *cur, omega, 1);
             if (rc) return rc;
         }
         return PS_OK;
@@ -200,22 +213,22 @@ int run_sweeps_untimed(ps_ctx *c, const double *rhs, double *p, double omega, in
         if ((long long)n * 2 * (long long)blocks > 0x7fffffffLL) return PS_EINVAL;
         ps::Grid g = c->g;
         const double *ax = c->ax, *ay = c->ay, *az = c->az;
-        unsigned *ctr = (unsigned *)c->done;
+        double *pp = *cur;
+        unsigned *ctr = c->ctr;
         if (blocks > 1) PS_CUDA(cudaMemsetAsync(ctr, 0, sizeof(unsigned), c->stream));
-        void *args[] = {&g, &ax, &ay, &az, &rhs, &p, &omega, &n, &ctr};
+        void *args[] = {&g, &ax, &ay, &az, &rhs, &pp, &omega, &n, &ctr};
         PS_CUDA(cudaLaunchCooperativeKernel((const void *)ps::ps_resident_sweeps_kernel,
                                             dim3((unsigned)blocks), dim3((unsigned)threads), args,
                                             0, c->stream));
         c->launches++;
         return PS_OK;
     }
-    double *src = p, *dst = c->p_alt;
-    int left = n;
+    double *src = *cur, *dst = (src == p) ? c->p_alt : p;
     const bool otf = c->variant == PS_KERNEL_FUSED_OTF;
     if (otf && !c->have_rho) return PS_ESTATE;
     const double c2x = 2.0 * (1.0 / (c->dx * c->dx)), c2y = 2.0 * (1.0 / (c->dy * c->dy)),
                  c2z = 2.0 * (1.0 / (c->dz * c->dz));
-    while (left > 0) {
+    for (int left = n; left > 0; --left) {
         cudaError_t e =
             otf ? ps::zm_launch_otf(c->fused, c->g, c->rho, c2x, c2y, c2z, rhs, src, dst, omega,
                                     c->stream)
@@ -223,19 +236,36 @@ int run_sweeps_untimed(ps_ctx *c, const double *rhs, double *p, double omega, in
                                 c->stream);
         c->launches++;
         if (e != cudaSuccess) return cuda_fail(e);
-        left -= 1;
         double *t = src; src = dst; dst = t;
     }
-    if (src != p) {
-        PS_CUDA(cudaMemcpyAsync(p, src, c->g.cells() * sizeof(double), cudaMemcpyDeviceToDevice,
+    *cur = src;
+    return PS_OK;
+}
+
+// Bring the iterate back into the caller's p if the ping-pong left it in p_alt.
+int settle_p(ps_ctx *c, double *p, double **cur)
+{
+    if (*cur != p) {
+        PS_CUDA(cudaMemcpyAsync(p, *cur, c->g.cells() * sizeof(double), cudaMemcpyDeviceToDevice,
                                 c->stream));
+        *cur = p;
     }
     return PS_OK;
 }
 
-int enqueue_residual(ps_ctx *c, const double *rhs, const double *p, double tol)
+// n sweeps in place on the caller's p (one device copy at the end if the ping-pong count is odd)
+int run_sweeps_inplace(ps_ctx *c, const double *rhs, double *p, double omega, int n)
 {
-    if (c->g.nx % 2 == 0 && (((uintptr_t)rhs | (uintptr_t)p) & 15u) == 0)
+    double *cur = p;
+    const int rc = run_sweeps(c, rhs, p, &cur, omega, n);
+    return rc ? rc : settle_p(c, p, &cur);
+}
+
+int enqueue_residual(ps_ctx *c, const double *rhs, const double *p)
+{
+    // the summation tree is a function of the grid shape alone (every *_dev pointer is 16-byte
+    // aligned: checked at the ABI), so the norm of given data never depends on where it lives
+    if (c->g.nx % 2 == 0)
         ps::ps_residual_partial_pair_kernel<<<c->nparts, ps::RED_THREADS, 0, c->stream>>>(
             c->g, c->ax, c->ay, c->az, rhs, p, c->partR2, c->partB2);
     else
@@ -244,8 +274,7 @@ int enqueue_residual(ps_ctx *c, const double *rhs, const double *p, double tol)
     c->launches++;
     PS_CUDA(cudaGetLastError());
     ps::ps_reduce_final_kernel<<<1, ps::FIN_THREADS, 0, c->stream>>>(c->partR2, c->partB2,
-                                                                    c->nparts, tol, c->scal,
-                                                                    nullptr);
+                                                                    c->nparts, c->scal);
     c->launches++;
     PS_CUDA(cudaGetLastError());
     PS_CUDA(cudaMemcpyAsync(c->h_scal, c->scal, 3 * sizeof(double), cudaMemcpyDeviceToHost,
@@ -274,13 +303,14 @@ int ps_create(ps_ctx **out, int nx, int ny, int nz, double dx, double dy, double
     ps_ctx *c = new (std::nothrow) ps_ctx();
     if (!c) return PS_ENOMEM;
     c->g = ps::Grid{nx, ny, nz};
+    c->device = dev;
     c->ev = new (std::nothrow) std::vector<cudaEvent_t>();
     if (!c->ev) { delete c; return PS_ENOMEM; }
     c->dx = dx; c->dy = dy; c->dz = dz;
     c->K = 50;
     c->sm_count = sms;
     c->coop = coop;
-    c->nparts = (int)((c->g.cells() + ps::RED_CHUNK - 1) / ps::RED_CHUNK);
+    c->nparts = nparts_for(c->g.cells());
     cudaError_t e = cudaMallocHost((void **)&c->h_scal, 4 * sizeof(double));
     if (e != cudaSuccess) { delete c->ev; delete c; return cuda_fail(e); }
     e = ps::zm_plan_init(&c->fused, c->g, sms);
@@ -301,14 +331,11 @@ int ps_destroy(ps_ctx *c)
 {
     if (!c) return PS_OK;
     if (c->child) ps_destroy(c->child);
-    if (c->lv_rhs) cudaFree(c->lv_rhs);
-    if (c->lv_p) cudaFree(c->lv_p);
+    if (c->mg_ws && c->mg_ws_owned) cudaFree(c->mg_ws);
     if (c->ws && c->ws_owned) cudaFree(c->ws);
     if (c->h_scal) cudaFreeHost(c->h_scal);
     ps::zm_plan_destroy(&c->fused);
-    if (c->st_F) cudaFree(c->st_F);
-    if (c->st_rhs) cudaFree(c->st_rhs);
-    if (c->st_p) cudaFree(c->st_p);
+    if (c->st_F && c->st_owned) cudaFree(c->st_F);
     if (c->ev) {
         for (cudaEvent_t e : *c->ev) cudaEventDestroy(e);
         delete c->ev;
@@ -329,6 +356,7 @@ int ps_set_workspace(ps_ctx *c, void *ws_dev, size_t bytes)
     c->ws_owned = false;
     c->have_coef = false;
     c->have_rho = false;
+    c->mg_ready = false;
     carve(c, ws_dev);
     return PS_OK;
 }
@@ -384,13 +412,13 @@ int ps_get_tuning(const ps_ctx *c, int *rows_per_thread, int *z_chunks, int *til
 
 int ps_set_fraction(ps_ctx *c, const double *F_dev, double rho_l, double rho_g)
 {
-    if (!c || !F_dev) return PS_EINVAL;
+    if (!c || !F_dev || !aligned16(F_dev)) return PS_EINVAL;
     if (!(rho_l > 0.0) || !(rho_g > 0.0) || !std::isfinite(rho_l) || !std::isfinite(rho_g))
         return PS_EINVAL;
     int rc = ensure_workspace(c);
     if (rc) return rc;
     const double cx = 1.0 / (c->dx * c->dx), cy = 1.0 / (c->dy * c->dy), cz = 1.0 / (c->dz * c->dz);
-    if (c->g.nx % 2 == 0 && ((uintptr_t)F_dev & 15u) == 0)
+    if (c->g.nx % 2 == 0)
         ps::ps_coef_build_pair_kernel<<<grid_for(c, c->g.cells() / 2, 256), 256, 0, c->stream>>>(
             c->g, cx, cy, cz, rho_l, rho_g, F_dev, c->ax, c->ay, c->az);
     else
@@ -424,16 +452,16 @@ int ps_export_coefficients(ps_ctx *c, double *ax_dev, double *ay_dev, double *az
 
 int ps_sweeps(ps_ctx *c, const double *rhs_dev, double *p_dev, double omega, int n)
 {
-    if (!c || !rhs_dev || !p_dev || n < 0) return PS_EINVAL;
+    if (!c || !rhs_dev || !p_dev || n < 0 || !aligned16(rhs_dev, p_dev)) return PS_EINVAL;
     if (!(omega > 0.0 && omega < 2.0)) return PS_EINVAL;
     if (!c->have_coef) return PS_ESTATE;
-    return run_sweeps(c, rhs_dev, p_dev, omega, n);
+    return run_sweeps_inplace(c, rhs_dev, p_dev, omega, n);
 }
 
 int ps_half_sweep(ps_ctx *c, const double *rhs_dev, double *p_dev, double omega, int colour)
 {
     if (!c || !rhs_dev || !p_dev || (colour != 0 && colour != 1)) return PS_EINVAL;
-    if (!(omega > 0.0 && omega < 2.0)) return PS_EINVAL;
+    if (!aligned16(rhs_dev, p_dev) || !(omega > 0.0 && omega < 2.0)) return PS_EINVAL;
     if (!c->have_coef) return PS_ESTATE;
     return launch_half_sweep(c, rhs_dev, p_dev, omega, colour);
 }
@@ -441,9 +469,9 @@ int ps_half_sweep(ps_ctx *c, const double *rhs_dev, double *p_dev, double omega,
 int ps_residual(ps_ctx *c, const double *rhs_dev, const double *p_dev, double *res_abs,
                 double *res_rel, double *rhs_norm)
 {
-    if (!c || !rhs_dev || !p_dev || !res_abs) return PS_EINVAL;
+    if (!c || !rhs_dev || !p_dev || !res_abs || !aligned16(rhs_dev, p_dev)) return PS_EINVAL;
     if (!c->have_coef) return PS_ESTATE;
-    int rc = enqueue_residual(c, rhs_dev, p_dev, 0.0);
+    int rc = enqueue_residual(c, rhs_dev, p_dev);
     if (rc) return rc;
     PS_CUDA(cudaStreamSynchronize(c->stream));
     *res_abs = c->h_scal[0];
@@ -455,34 +483,41 @@ int ps_residual(ps_ctx *c, const double *rhs_dev, const double *p_dev, double *r
 int ps_solve(ps_ctx *c, const double *rhs_dev, double *p_dev, double omega, int max_sweeps,
              double tol, ps_info *info)
 {
-    if (!c || !rhs_dev || !p_dev || max_sweeps < 0) return PS_EINVAL;
+    if (!c || !rhs_dev || !p_dev || max_sweeps < 0 || !aligned16(rhs_dev, p_dev)) return PS_EINVAL;
     if (!(omega > 0.0 && omega < 2.0)) return PS_EINVAL;
     if (!c->have_coef) return PS_ESTATE;
     int s = 0, converged = 0, rc = 0;
     bool checked = false;
+    // the fused kernels ping-pong between p_dev and p_alt; the checks read whichever buffer holds
+    // the iterate, and p_dev is brought up to date once, at the end (no copy per odd batch)
+    double *cur = p_dev;
     if (tol > 0.0) {
         while (s < max_sweeps) {
             const int batch = (max_sweeps - s < c->K) ? (max_sweeps - s) : c->K;   // next check
-            rc = run_sweeps(c, rhs_dev, p_dev, omega, batch);
+            rc = run_sweeps(c, rhs_dev, p_dev, &cur, omega, batch);
             if (rc) return rc;
             s += batch;
-            rc = enqueue_residual(c, rhs_dev, p_dev, tol);
+            rc = enqueue_residual(c, rhs_dev, cur);
             if (rc) return rc;
             PS_CUDA(cudaStreamSynchronize(c->stream));
             checked = true;
             if (c->h_scal[1] <= tol) { converged = 1; break; }
         }
     } else {
-        rc = run_sweeps(c, rhs_dev, p_dev, omega, max_sweeps);
+        rc = run_sweeps(c, rhs_dev, p_dev, &cur, omega, max_sweeps);
         if (rc) return rc;
         s = max_sweeps;
     }
+    if ((rc = settle_p(c, p_dev, &cur))) return rc;
     if (!checked) {
-        rc = enqueue_residual(c, rhs_dev, p_dev, tol);
+        rc = enqueue_residual(c, rhs_dev, p_dev);
         if (rc) return rc;
-        PS_CUDA(cudaStreamSynchronize(c->stream));
-        if (tol > 0.0 && c->h_scal[1] <= tol) converged = 1;
+        if (tol > 0.0) {
+            PS_CUDA(cudaStreamSynchronize(c->stream));
+            if (c->h_scal[1] <= tol) converged = 1;
+        }
     }
+    PS_CUDA(cudaStreamSynchronize(c->stream));
     if (info) {
         info->sweeps = s;
         info->converged = converged;
@@ -493,6 +528,20 @@ int ps_solve(ps_ctx *c, const double *rhs_dev, double *p_dev, double omega, int 
     return PS_OK;
 }
 
+size_t ps_host_staging_bytes(const ps_ctx *c) { return c ? 3 * field_bytes(c) : 0; }
+
+int ps_set_host_staging(ps_ctx *c, void *st_dev, size_t bytes)
+{
+    if (!c || !st_dev) return PS_EINVAL;
+    if (((uintptr_t)st_dev & 255u) != 0 || bytes < 3 * field_bytes(c)) return PS_EINVAL;
+    if (c->st_F && c->st_owned) cudaFree(c->st_F);
+    c->st_F = (double *)st_dev;
+    c->st_rhs = (double *)((char *)st_dev + field_bytes(c));
+    c->st_p = (double *)((char *)st_dev + 2 * field_bytes(c));
+    c->st_owned = false;
+    return PS_OK;
+}
+
 int ps_solve_host(ps_ctx *c, const double *F_host, double rho_l, double rho_g,
                   const double *rhs_host, double *p_host, double omega, int max_sweeps,
                   double tol, ps_info *info)
@@ -500,22 +549,20 @@ int ps_solve_host(ps_ctx *c, const double *F_host, double rho_l, double rho_g,
     if (!c || !F_host || !rhs_host || !p_host) return PS_EINVAL;
     const size_t b = c->g.cells() * sizeof(double);
     if (!c->st_F) {
-        cudaError_t e = cudaMalloc((void **)&c->st_F, b);
-        if (e == cudaSuccess) e = cudaMalloc((void **)&c->st_rhs, b);
-        if (e == cudaSuccess) e = cudaMalloc((void **)&c->st_p, b);
+        void *st = nullptr;
+        const cudaError_t e = cudaMalloc(&st, 3 * field_bytes(c));
         if (e != cudaSuccess) {
             cudaGetLastError();
-            if (c->st_F) cudaFree(c->st_F);
-            if (c->st_rhs) cudaFree(c->st_rhs);
-            c->st_F = c->st_rhs = c->st_p = nullptr;
             return e == cudaErrorMemoryAllocation ? PS_ENOMEM : cuda_fail(e);
         }
+        ps_set_host_staging(c, st, 3 * field_bytes(c));
+        c->st_owned = true;
     }
     PS_CUDA(cudaMemcpyAsync(c->st_F, F_host, b, cudaMemcpyHostToDevice, c->stream));
-    PS_CUDA(cudaMemcpyAsync(c->st_rhs, rhs_host, b, cudaMemcpyHostToDevice, c->stream));
-    PS_CUDA(cudaMemcpyAsync(c->st_p, p_host, b, cudaMemcpyHostToDevice, c->stream));
     int rc = ps_set_fraction(c, c->st_F, rho_l, rho_g);
     if (rc) return rc;
+    PS_CUDA(cudaMemcpyAsync(c->st_rhs, rhs_host, b, cudaMemcpyHostToDevice, c->stream));
+    PS_CUDA(cudaMemcpyAsync(c->st_p, p_host, b, cudaMemcpyHostToDevice, c->stream));
     rc = ps_solve(c, c->st_rhs, c->st_p, omega, max_sweeps, tol, info);
     if (rc) return rc;
     PS_CUDA(cudaMemcpyAsync(p_host, c->st_p, b, cudaMemcpyDeviceToHost, c->stream));
@@ -530,7 +577,7 @@ int ps_enable_timing(ps_ctx *c, int on)
     return PS_OK;
 }
 
-int ps_timing(ps_ctx *c, double *sweep_ms, long long *sweep_launches)
+int ps_timing(ps_ctx *c, double *sweep_ms, long long *sweep_launches, long long *sweeps)
 {
     if (!c) return PS_EINVAL;
     PS_CUDA(cudaStreamSynchronize(c->stream));
@@ -542,8 +589,10 @@ int ps_timing(ps_ctx *c, double *sweep_ms, long long *sweep_launches)
     }
     if (sweep_ms) *sweep_ms = tot;
     if (sweep_launches) *sweep_launches = c->timed_launches;
+    if (sweeps) *sweeps = c->timed_sweeps;
     c->ev_used = 0;
     c->timed_launches = 0;
+    c->timed_sweeps = 0;
     return PS_OK;
 }
 
@@ -568,8 +617,69 @@ int mg_max_levels(int nx, int ny, int nz)
     return L;
 }
 
+// device bytes of the coarse levels 1 .. nlev-1 of a hierarchy on grid g: per level the context's
+// own workspace (coefficients, ping-pong buffer, partials) + its right-hand side + its correction
+size_t mg_bytes(ps::Grid g, int nlev)
+{
+    size_t tot = 0;
+    for (int l = 1; l < nlev; ++l) {
+        g = ps::Grid{g.nx / 2, g.ny / 2, g.nz / 2};
+        tot += workspace_bytes_for(g.cells()) + 2 * field_bytes_for(g.cells());
+    }
+    return tot;
+}
+
+void mg_drop_levels(ps_ctx *c)
+{
+    if (c->child) ps_destroy(c->child);
+    c->child = nullptr;
+    c->mg_nlev = 0;
+    c->mg_ready = false;
+}
+
+// Create the contexts of levels 1 .. nlev-1 below c and hand each its slice of the level block
+// (the caller's ps_mg_set_workspace block, else one cudaMalloc owned by c).
+int mg_build_levels(ps_ctx *c, int nlev)
+{
+    const size_t need = mg_bytes(c->g, nlev);
+    if (need > 0) {
+        if (c->mg_ws && !c->mg_ws_owned && c->mg_ws_bytes < need) return PS_EINVAL;
+        if (c->mg_ws && c->mg_ws_owned && c->mg_ws_bytes < need) {
+            cudaFree(c->mg_ws);
+            c->mg_ws = nullptr;
+        }
+        if (!c->mg_ws) {
+            const cudaError_t e = cudaMalloc(&c->mg_ws, need);
+            if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); c->mg_ws = nullptr; return PS_ENOMEM; }
+            if (e != cudaSuccess) { c->mg_ws = nullptr; return cuda_fail(e); }
+            c->mg_ws_bytes = need;
+            c->mg_ws_owned = true;
+        }
+    }
+    char *q = (char *)c->mg_ws;
+    ps_ctx *f = c;
+    for (int l = 1; l < nlev; ++l) {
+        ps_ctx *k = nullptr;
+        int rc = ps_create(&k, f->g.nx / 2, f->g.ny / 2, f->g.nz / 2, 2.0 * f->dx, 2.0 * f->dy,
+                           2.0 * f->dz);
+        if (rc) return rc;
+        f->child = k;
+        if ((rc = ps_set_workspace(k, q, workspace_bytes(k)))) return rc;
+        q += workspace_bytes(k);
+        k->lv_rhs = (double *)q; q += field_bytes(k);
+        k->lv_p = (double *)q; q += field_bytes(k);
+        f = k;
+    }
+    return PS_OK;
+}
+
 int mg_launch_coarsen(ps_ctx *f, ps_ctx *k)
 {
+    const char *exp_ = getenv("PS_EXP_COARSEN");
+    if (exp_ && exp_[0] == '1')
+        ps::ps_mg_coarsen_series_kernel<<<grid_for(f, k->g.cells(), 256), 256, 0, f->stream>>>(
+            f->g, f->ax, f->ay, f->az, k->ax, k->ay, k->az);
+    else
     ps::ps_mg_coarsen_kernel<<<grid_for(f, k->g.cells(), 256), 256, 0, f->stream>>>(
         f->g, f->ax, f->ay, f->az, k->ax, k->ay, k->az);
     f->launches++;
@@ -580,12 +690,8 @@ int mg_launch_coarsen(ps_ctx *f, ps_ctx *k)
 
 int mg_launch_residual_restrict(ps_ctx *f, const double *rhs, const double *p, double *rc)
 {
-    if ((((uintptr_t)rhs | (uintptr_t)p) & 15u) == 0)
-        ps::ps_mg_residual_restrict_pair_kernel<<<grid_for(f, f->g.cells() / 8, 256), 256, 0,
-                                                  f->stream>>>(f->g, f->ax, f->ay, f->az, rhs, p, rc);
-    else
-        ps::ps_mg_residual_restrict_kernel<<<grid_for(f, f->g.cells() / 8, 256), 256, 0,
-                                             f->stream>>>(f->g, f->ax, f->ay, f->az, rhs, p, rc);
+    ps::ps_mg_residual_restrict_pair_kernel<<<grid_for(f, f->g.cells() / 8, 256), 256, 0,
+                                              f->stream>>>(f->g, f->ax, f->ay, f->az, rhs, p, rc);
     f->launches++;
     PS_CUDA(cudaGetLastError());
     return PS_OK;
@@ -609,24 +715,21 @@ int mg_nu(int nu, int level, const ps_mg_params &m)
 
 // The finest level of ps_mg_solve may take its norm inside the residual + restriction pass: with
 // no pre-smoothing there (nu1 = 0) the residual that is restricted is the residual of the
-// iterate the stopping test looks at.  Needs the pair kernel's preconditions.
-bool mg_fused_norm_ok(const ps_ctx *f, const double *rhs, const double *p)
+// iterate the stopping test looks at.
+bool mg_fused_norm_ok(const ps_ctx *f)
 {
-    return f->child && f->mg_nlev > 1 && mg_nu(f->mgp.nu1, 0, f->mgp) == 0 && f->g.nx % 2 == 0 &&
-           aligned16(rhs, p);
+    return f->child && f->mg_nlev > 1 && mg_nu(f->mgp.nu1, 0, f->mgp) == 0;
 }
 
 // residual + restriction + norm partials of level f, then the final reduction and the read-back
-int mg_launch_residual_restrict_norm(ps_ctx *f, const double *rhs, const double *p, double *rc,
-                                     double tol)
+int mg_launch_residual_restrict_norm(ps_ctx *f, const double *rhs, const double *p, double *rc)
 {
     ps::ps_mg_residual_restrict_norm_kernel<<<f->nparts, ps::RED_THREADS, 0, f->stream>>>(
         f->g, f->ax, f->ay, f->az, rhs, p, rc, f->partR2, f->partB2);
     f->launches++;
     PS_CUDA(cudaGetLastError());
     ps::ps_reduce_final_kernel<<<1, ps::FIN_THREADS, 0, f->stream>>>(f->partR2, f->partB2,
-                                                                    f->nparts, tol, f->scal,
-                                                                    nullptr);
+                                                                    f->nparts, f->scal);
     f->launches++;
     PS_CUDA(cudaGetLastError());
     PS_CUDA(cudaMemcpyAsync(f->h_scal, f->scal, 3 * sizeof(double), cudaMemcpyDeviceToHost,
@@ -641,22 +744,41 @@ int mg_cycle(ps_ctx *f, const ps_mg_params &m, const double *rhs, double *p, int
 {
     int rc;
     if (!f->child || f->mg_nlev <= 1)
-        return run_sweeps(f, rhs, p, m.omega_s, m.coarse_sweeps);
+        return run_sweeps_inplace(f, rhs, p, m.omega_s, m.coarse_sweeps);
     ps_ctx *k = f->child;
     if (!restricted) {
-        if ((rc = run_sweeps(f, rhs, p, m.omega_s, mg_nu(m.nu1, level, m)))) return rc;
+        if ((rc = run_sweeps_inplace(f, rhs, p, m.omega_s, mg_nu(m.nu1, level, m)))) return rc;
         if ((rc = mg_launch_residual_restrict(f, rhs, p, k->lv_rhs))) return rc;
     }
     PS_CUDA(cudaMemsetAsync(k->lv_p, 0, k->g.cells() * sizeof(double), f->stream));
     for (int g = 0; g < m.gamma; ++g)
         if ((rc = mg_cycle(k, m, k->lv_rhs, k->lv_p, level + 1))) return rc;
     if ((rc = mg_launch_prolong_add(f, k->lv_p, p))) return rc;
-    return run_sweeps(f, rhs, p, m.omega_s, mg_nu(m.nu2, level, m));
+    return run_sweeps_inplace(f, rhs, p, m.omega_s, mg_nu(m.nu2, level, m));
 }
 
 }  // namespace
 
 extern "C" {
+
+size_t ps_mg_workspace_bytes(const ps_ctx *c, int levels)
+{
+    if (!c) return 0;
+    const int maxl = mg_max_levels(c->g.nx, c->g.ny, c->g.nz);
+    const int nlev = levels > maxl ? maxl : (levels < 1 ? 1 : levels);
+    return mg_bytes(c->g, nlev);
+}
+
+int ps_mg_set_workspace(ps_ctx *c, void *ws_dev, size_t bytes)
+{
+    if (!c || !ws_dev || ((uintptr_t)ws_dev & 255u) != 0) return PS_EINVAL;
+    mg_drop_levels(c);                       // the old levels point into the old block
+    if (c->mg_ws && c->mg_ws_owned) cudaFree(c->mg_ws);
+    c->mg_ws = ws_dev;
+    c->mg_ws_bytes = bytes;
+    c->mg_ws_owned = false;
+    return PS_OK;
+}
 
 int ps_mg_setup(ps_ctx *c, const ps_mg_params *prm)
 {
@@ -666,32 +788,24 @@ int ps_mg_setup(ps_ctx *c, const ps_mg_params *prm)
         prm->gamma > 2 || !(prm->omega_s > 0.0 && prm->omega_s < 2.0))
         return PS_EINVAL;
     if (!c->have_coef) return PS_ESTATE;
+    int dev = -1;
+    PS_CUDA(cudaGetDevice(&dev));
+    if (dev != c->device) return PS_EINVAL;    // the levels must live on the context's device
+    c->mg_ready = false;
     int nlev = prm->levels;
     const int maxl = mg_max_levels(c->g.nx, c->g.ny, c->g.nz);
     if (nlev > maxl) nlev = maxl;
     if (nlev < 1) nlev = 1;
-    if (c->mg_nlev != nlev && c->child) {          // different depth: rebuild the chain
-        ps_destroy(c->child);
-        c->child = nullptr;
+    if (c->mg_nlev != nlev) {                  // first set-up or another depth: (re)build the chain
+        mg_drop_levels(c);
+        const int rc = mg_build_levels(c, nlev);
+        if (rc) { mg_drop_levels(c); return rc; }
     }
     ps_ctx *f = c;
     for (int l = 0; l < nlev; ++l) {
         f->mg_nlev = nlev - l;
         f->mgp = *prm;
         if (l == nlev - 1) break;
-        if (!f->child) {
-            ps_ctx *k = nullptr;
-            int rc = ps_create(&k, f->g.nx / 2, f->g.ny / 2, f->g.nz / 2, 2.0 * f->dx, 2.0 * f->dy,
-                               2.0 * f->dz);
-            if (rc) return rc;
-            f->child = k;
-            if ((rc = ensure_workspace(k))) return rc;
-            const size_t b = k->g.cells() * sizeof(double);
-            cudaError_t e = cudaMalloc((void **)&k->lv_rhs, b);
-            if (e == cudaSuccess) e = cudaMalloc((void **)&k->lv_p, b);
-            if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); return PS_ENOMEM; }
-            if (e != cudaSuccess) return cuda_fail(e);
-        }
         f->child->stream = c->stream;
         const int rc = mg_launch_coarsen(f, f->child);
         if (rc) return rc;
@@ -706,16 +820,16 @@ int ps_mg_levels(const ps_ctx *c) { return c ? c->mg_nlev : 0; }
 int ps_mg_solve(ps_ctx *c, const double *rhs_dev, double *p_dev, int max_cycles, double tol,
                 ps_info *info)
 {
-    if (!c || !rhs_dev || !p_dev || max_cycles < 0) return PS_EINVAL;
+    if (!c || !rhs_dev || !p_dev || max_cycles < 0 || !aligned16(rhs_dev, p_dev)) return PS_EINVAL;
     if (!c->have_coef || !c->mg_ready) return PS_ESTATE;
     for (ps_ctx *k = c->child; k; k = k->child) k->stream = c->stream;
     int cyc = 0, converged = 0, rc = 0;
-    if (mg_fused_norm_ok(c, rhs_dev, p_dev) && max_cycles > 0) {
+    if (mg_fused_norm_ok(c) && max_cycles > 0) {
         // (cycle, check)* as below, but the check of cycle n rides on the residual + restriction
         // pass that opens cycle n + 1 (one pass of 41 B/cell instead of 40 + 41); the pass after
         // the last cycle only serves the norm
         for (cyc = 0;; ++cyc) {
-            if ((rc = mg_launch_residual_restrict_norm(c, rhs_dev, p_dev, c->child->lv_rhs, tol)))
+            if ((rc = mg_launch_residual_restrict_norm(c, rhs_dev, p_dev, c->child->lv_rhs)))
                 return rc;
             if (cyc >= 1) {
                 PS_CUDA(cudaStreamSynchronize(c->stream));
@@ -735,14 +849,14 @@ int ps_mg_solve(ps_ctx *c, const double *rhs_dev, double *p_dev, int max_cycles,
     }
     for (cyc = 1; cyc <= max_cycles; ++cyc) {
         if ((rc = mg_cycle(c, c->mgp, rhs_dev, p_dev))) return rc;
-        if ((rc = enqueue_residual(c, rhs_dev, p_dev, tol))) return rc;
+        if ((rc = enqueue_residual(c, rhs_dev, p_dev))) return rc;
         PS_CUDA(cudaStreamSynchronize(c->stream));
         if (tol > 0.0 && c->h_scal[1] <= tol) { converged = 1; break; }
         if (!std::isfinite(c->h_scal[1])) break;
     }
     if (cyc > max_cycles) cyc = max_cycles;
     if (max_cycles == 0) {
-        if ((rc = enqueue_residual(c, rhs_dev, p_dev, tol))) return rc;
+        if ((rc = enqueue_residual(c, rhs_dev, p_dev))) return rc;
         PS_CUDA(cudaStreamSynchronize(c->stream));
     }
     if (info) {
@@ -768,7 +882,7 @@ int ps_mg_export_coarse(ps_ctx *c, int level, double *ax_dev, double *ay_dev, do
 
 int ps_mg_residual_restrict(ps_ctx *c, const double *rhs_dev, const double *p_dev, double *rc_dev)
 {
-    if (!c || !rhs_dev || !p_dev || !rc_dev) return PS_EINVAL;
+    if (!c || !rhs_dev || !p_dev || !rc_dev || !aligned16(rhs_dev, p_dev)) return PS_EINVAL;
     if (!c->have_coef) return PS_ESTATE;
     if (c->g.nx % 2 || c->g.ny % 2 || c->g.nz % 2) return PS_EINVAL;
     return mg_launch_residual_restrict(c, rhs_dev, p_dev, rc_dev);
@@ -776,7 +890,7 @@ int ps_mg_residual_restrict(ps_ctx *c, const double *rhs_dev, const double *p_de
 
 int ps_mg_prolong_add(ps_ctx *c, const double *ec_dev, double *p_dev)
 {
-    if (!c || !ec_dev || !p_dev) return PS_EINVAL;
+    if (!c || !ec_dev || !p_dev || !aligned16(p_dev)) return PS_EINVAL;
     if (c->g.nx % 2 || c->g.ny % 2 || c->g.nz % 2) return PS_EINVAL;
     return mg_launch_prolong_add(c, ec_dev, p_dev);
 }
@@ -790,8 +904,9 @@ int ps_rhs_from_velocity(ps_ctx *c, const double *ux_dev, const double *uy_dev,
 {
     if (!c || !ux_dev || !uy_dev || !uz_dev || !rhs_dev) return PS_EINVAL;
     if (!(dt > 0.0) || !std::isfinite(dt)) return PS_EINVAL;
+    if (!aligned16(ux_dev, uy_dev, uz_dev, rhs_dev)) return PS_EINVAL;
     const ps::Spacing h{c->dx, c->dy, c->dz};
-    if (c->g.nx % 2 == 0 && aligned16(ux_dev, uy_dev, uz_dev, rhs_dev))
+    if (c->g.nx % 2 == 0)
         ps::ps_rhs_from_velocity_pair_kernel<<<grid_for(c, c->g.cells() / 2, 256), 256, 0,
                                                c->stream>>>(c->g, h, ux_dev, uy_dev, uz_dev, dt,
                                                             rhs_dev);
@@ -808,6 +923,7 @@ int ps_correct_velocity(ps_ctx *c, const double *p_dev, double dt, double *ux_de
 {
     if (!c || !p_dev || !ux_dev || !uy_dev || !uz_dev) return PS_EINVAL;
     if (!(dt > 0.0) || !std::isfinite(dt)) return PS_EINVAL;
+    if (!aligned16(p_dev, ux_dev, uy_dev, uz_dev)) return PS_EINVAL;
     if (!c->have_coef) return PS_ESTATE;
     const ps::Spacing h{c->dx, c->dy, c->dz};
     ps::ps_correct_velocity_kernel<<<grid_for(c, c->g.cells(), 256), 256, 0, c->stream>>>(
@@ -822,9 +938,10 @@ int ps_face_divergence(ps_ctx *c, const double *ux_dev, const double *uy_dev, co
 {
     if (!c || !ux_dev || !uy_dev || !uz_dev || !p_dev || !div_dev) return PS_EINVAL;
     if (!(dt > 0.0) || !std::isfinite(dt)) return PS_EINVAL;
+    if (!aligned16(ux_dev, uy_dev, uz_dev, p_dev) || !aligned16(div_dev)) return PS_EINVAL;
     if (!c->have_coef) return PS_ESTATE;
     const ps::Spacing h{c->dx, c->dy, c->dz};
-    if (c->g.nx % 2 == 0 && aligned16(ux_dev, uy_dev, uz_dev, p_dev) && aligned16(div_dev))
+    if (c->g.nx % 2 == 0)
         ps::ps_face_divergence_pair_kernel<<<grid_for(c, c->g.cells() / 2, 256), 256, 0,
                                              c->stream>>>(c->g, h, c->ax, c->ay, c->az, ux_dev,
                                                           uy_dev, uz_dev, p_dev, dt, div_dev);
@@ -840,8 +957,9 @@ int ps_ssf_rhs(ps_ctx *c, const double *F_dev, const double *kappa_dev, double s
                double *rhs_dev)
 {
     if (!c || !F_dev || !kappa_dev || !rhs_dev || !std::isfinite(sigma)) return PS_EINVAL;
+    if (!aligned16(F_dev, kappa_dev, rhs_dev)) return PS_EINVAL;
     if (!c->have_coef) return PS_ESTATE;
-    if (c->g.nx % 2 == 0 && aligned16(F_dev, kappa_dev, rhs_dev))
+    if (c->g.nx % 2 == 0)
         ps::ps_ssf_rhs_pair_kernel<<<grid_for(c, c->g.cells() / 2, 256), 256, 0, c->stream>>>(
             c->g, c->ax, c->ay, c->az, F_dev, kappa_dev, sigma, rhs_dev);
     else

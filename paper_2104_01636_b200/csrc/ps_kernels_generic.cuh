@@ -7,8 +7,8 @@
 // These work for any nx, ny >= 1 and even nz >= 2 and are the reference schedule of the CUDA
 // path: one thread per cell (coefficients, residual) or per cell of the active colour (sweep),
 // plain coalesced global loads, neighbour reuse left to L1/L2.  The fast kernels of
-// ps_kernels_fused.cuh compute the same expressions in the same order, so every variant gives
-// bitwise identical p.  Compile with --fmad=false: every * and + below rounds separately.
+// ps_kernels_zmarch.cuh and ps_kernels_resident.cuh compute the same expressions in the same
+// order, so every variant gives bitwise identical p.  Compile with --fmad=false: every * and + below rounds separately.
 #pragma once
 #include <cstddef>
 #include <cstdint>
@@ -293,7 +293,7 @@ ps_residual_partial_kernel(Grid g, const double *__restrict__ ax, const double *
     }
 }
 
-// The same for even nx and 16-byte aligned rhs, p: thread t takes the x-pairs t, t+256, ... of the
+// The same for even nx (every ABI pointer is 16-byte aligned): thread t takes the x-pairs t, t+256, ... of the
 // block's chunk (left cell first).  A different but equally fixed summation tree.
 __global__ void __launch_bounds__(RED_THREADS)
 ps_residual_partial_pair_kernel(Grid g, const double *__restrict__ ax,
@@ -331,13 +331,11 @@ ps_residual_partial_pair_kernel(Grid g, const double *__restrict__ ax,
 
 // Pass 2: one block; thread t adds partials t, t+1024, ... in order, then the same fixed tree.
 // out[0] = ||r||_2, out[1] = ||r||_2/||rhs||_2 (||r||_2 if rhs == 0), out[2] = ||rhs||_2.
-// If tol > 0 and out[1] <= tol the device flag done[0] is raised (sweep kernels launched after
-// it may then return at once; see ps_api.cu).
 constexpr int FIN_THREADS = 1024;
 
 __global__ void __launch_bounds__(FIN_THREADS)
 ps_reduce_final_kernel(const double *__restrict__ partR2, const double *__restrict__ partB2,
-                       int nparts, double tol, double *__restrict__ out, int *done)
+                       int nparts, double *__restrict__ out)
 {
     __shared__ double sm[FIN_THREADS / 32];
     double r2 = 0.0, b2 = 0.0;
@@ -353,7 +351,6 @@ ps_reduce_final_kernel(const double *__restrict__ partR2, const double *__restri
         out[0] = ra;
         out[1] = rr;
         out[2] = bn;
-        if (done != nullptr && tol > 0.0 && rr <= tol) done[0] = 1;
     }
 }
 

@@ -15,7 +15,7 @@ import json
 import sys
 import time
 
-BYTES_PER_UPDATE = {"twopass": 80.0, "fused": 48.0, "resident": 80.0}
+BYTES_PER_UPDATE = {"twopass": 80.0, "fused": 48.0, "fused_otf": 32.0, "resident": 80.0}
 
 
 def run_config(cfg: int, max_sweeps: int, to_tol: bool, kernel: int, mg_cycles: int = 1000,
@@ -128,7 +128,7 @@ def main(argv=None):
     ap.add_argument("--no-tol", action="store_true", help="skip the to-tolerance solves")
     ap.add_argument("--mg-cycles", type=int, default=1000, help="cap of multigrid cycles")
     ap.add_argument("--sweeps", type=int, default=0, help="fixed-sweep count (default: the config's)")
-    ap.add_argument("--kernel", default="auto", choices=["auto", "twopass", "fused"])
+    ap.add_argument("--kernel", default="auto", choices=["auto", "twopass", "fused", "fused_otf"])
     ap.add_argument("--md", default="", help="also write the table to this file")
     ap.add_argument("--kernel-rates", action="store_true",
                     help="only time the single-pass kernels on config 4 and print their rates")
@@ -140,7 +140,7 @@ def main(argv=None):
     build.build()
     binding.load()
     kernel = {"auto": binding.KERNEL_AUTO, "twopass": binding.KERNEL_TWOPASS,
-              "fused": binding.KERNEL_FUSED}[args.kernel]
+              "fused": binding.KERNEL_FUSED, "fused_otf": binding.KERNEL_FUSED_OTF}[args.kernel]
     if args.kernel_rates:
         md = kernel_rates()
         print(md)

@@ -216,10 +216,11 @@ def test_config3_fixed_sweeps(torch_cuda, B, ora):
         assert abs(ig.res_rel - io.res_rel) <= NORM_TOL * io.res_rel
 
 
-@pytest.mark.parametrize("cfg,nsweeps", [(4, 500), (5, 24)])
+@pytest.mark.parametrize("cfg,nsweeps", [(4, 500), (5, 300)])
 def test_full_size_configs(torch_cuda, B, ora, cfg, nsweeps):
     """configs[3] (256x256x512, 864 spheres, its full 500 sweeps) and configs[4] (384x384x1024,
-    2048 spheres; 24 of its 300 sweeps -- what the oracle does in ~10 s) at full size in the launch
+    2048 spheres, its full 300 sweeps: 4.5e10 oracle updates, about a minute of host time) at full
+    size in the launch
     configuration bench.py times (kernel AUTO): full-field bitwise parity of p and the norms, then
     two properties that hold at any size: the norm ps_solve reports equals a fresh ps_residual,
     and rolling the inputs by an even number of z planes rolls p bitwise (pin P7)."""
@@ -483,3 +484,79 @@ def test_long_run_repeatable_across_fused_variants(torch_cuda, B):
                 ref = p_d.clone()
             else:
                 assert torch_cuda.equal(p_d, ref), (kernel, rpt, chunks)
+
+
+def test_unaligned_pointers_are_rejected_everywhere(torch_cuda, B, ora):
+    """Every *_dev field pointer must be 16-byte aligned (include/ps_poisson.h "Pointers").  A
+    contiguous view at an odd storage offset is 8-byte aligned only: each entry point must return
+    PS_EINVAL before launching anything (a 16-byte access or a TMA map on such a pointer would
+    fault and poison the CUDA context), the binding must refuse such a tensor, and the context must
+    work as before afterwards."""
+    import ctypes
+    w = shape_workload(40, 36, 24, 2, 8, None)
+    n = w.nx * w.ny * w.nz
+    shape = (w.nz, w.ny, w.nx)
+
+    def odd(a=None):
+        buf = torch_cuda.zeros(n + 1, dtype=torch_cuda.float64, device="cuda")
+        v = buf[1:].view(shape)
+        if a is not None:
+            v.copy_(to_dev(torch_cuda, a))
+        assert v.is_contiguous() and v.data_ptr() % 16 == 8
+        return v
+
+    coef = ora.coefficients(w.F, w.rho_l, w.rho_g, w.dx, w.dy, w.dz)
+    p_ora = np.zeros_like(w.rhs)
+    ora.sweep(coef, w.rhs, p_ora, w.omega, 3)
+    lib = B.load()
+    ptr = lambda t: ctypes.c_void_p(t.data_ptr())
+    for kernel in (B.KERNEL_TWOPASS, B.KERNEL_FUSED, B.KERNEL_RESIDENT):
+        with B.PoissonSolver(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz) as s:
+            s.set_kernel(kernel)
+            F_d, rhs_d = to_dev(torch_cuda, w.F), to_dev(torch_cuda, w.rhs)
+            p_d = torch_cuda.zeros_like(rhs_d)
+            bad_F, bad_rhs, bad_p = odd(w.F), odd(w.rhs), odd()
+            h = s._h
+            assert lib.ps_set_fraction(h, ptr(bad_F), w.rho_l, w.rho_g) == B.PS_EINVAL
+            s.set_fraction(F_d, w.rho_l, w.rho_g)
+            s.mg_setup(levels=2)
+            dbl = ctypes.c_double()
+            for rhs_t, p_t in ((bad_rhs, p_d), (rhs_d, bad_p), (bad_rhs, bad_p)):
+                assert lib.ps_sweeps(h, ptr(rhs_t), ptr(p_t), w.omega, 1) == B.PS_EINVAL
+                assert lib.ps_half_sweep(h, ptr(rhs_t), ptr(p_t), w.omega, 0) == B.PS_EINVAL
+                assert lib.ps_solve(h, ptr(rhs_t), ptr(p_t), w.omega, 1, 0.0, None) == B.PS_EINVAL
+                assert lib.ps_residual(h, ptr(rhs_t), ptr(p_t), ctypes.byref(dbl), None, None) == B.PS_EINVAL
+                assert lib.ps_mg_solve(h, ptr(rhs_t), ptr(p_t), 1, 0.0, None) == B.PS_EINVAL
+                assert lib.ps_mg_residual_restrict(h, ptr(rhs_t), ptr(p_t), ptr(p_d)) == B.PS_EINVAL
+            assert lib.ps_mg_prolong_add(h, ptr(rhs_d), ptr(bad_p)) == B.PS_EINVAL
+            assert lib.ps_rhs_from_velocity(h, ptr(bad_p), ptr(p_d), ptr(p_d), 1e-3, ptr(rhs_d)) == B.PS_EINVAL
+            assert lib.ps_correct_velocity(h, ptr(bad_p), 1e-3, ptr(p_d), ptr(p_d), ptr(p_d)) == B.PS_EINVAL
+            assert lib.ps_face_divergence(h, ptr(p_d), ptr(p_d), ptr(p_d), ptr(bad_p), 1e-3, ptr(rhs_d)) == B.PS_EINVAL
+            assert lib.ps_ssf_rhs(h, ptr(bad_F), ptr(F_d), 0.07, ptr(rhs_d)) == B.PS_EINVAL
+            with pytest.raises(TypeError, match="16-byte"):
+                s.sweeps(rhs_d, bad_p, w.omega, 1)
+            assert float(bad_p.abs().max()) == 0.0 and float(p_d.abs().max()) == 0.0   # untouched
+            s.sweeps(rhs_d, p_d, w.omega, 3)                      # the context is still healthy
+            assert_p_parity(p_d.cpu().numpy(), p_ora, f"after rejected calls, kernel {kernel}")
+
+
+def test_odd_check_interval_needs_no_copy_and_matches_oracle(torch_cuda, B, ora):
+    """K odd: the fused kernels end every batch in the other ping-pong buffer; ps_solve takes the
+    norm on whichever buffer holds the iterate and settles p once at the end.  Same stops, same p."""
+    w = shape_workload(72, 52, 34, 3, 12, None)
+    coef = ora.coefficients(w.F, w.rho_l, w.rho_g, w.dx, w.dy, w.dz)
+    for K, max_sweeps, tol in [(7, 64, 1e-30), (3, 40, 0.5), (5, 23, 1e-30), (1, 9, 1e-30)]:
+        p_ora = np.zeros_like(w.rhs)
+        io = ora.solve(coef, w.rhs, p_ora, w.omega, max_sweeps, tol, check_interval=K)
+        for kernel in (B.KERNEL_FUSED, B.KERNEL_FUSED_OTF, B.KERNEL_TWOPASS):
+            with B.PoissonSolver(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz) as s:
+                s.set_kernel(kernel)
+                s.set_check_interval(K)
+                s.set_fraction(to_dev(torch_cuda, w.F), w.rho_l, w.rho_g)
+                rhs_d = to_dev(torch_cuda, w.rhs)
+                p_d = torch_cuda.zeros_like(rhs_d)
+                ig = s.solve(rhs_d, p_d, w.omega, max_sweeps, tol)
+                assert (ig.sweeps, ig.converged) == (io.sweeps, io.converged), (K, max_sweeps, tol)
+                assert_p_parity(p_d.cpu().numpy(), p_ora, f"K={K} kernel {kernel}")
+                assert abs(ig.res_rel - io.res_rel) <= NORM_TOL * io.res_rel
+                assert s.residual(rhs_d, p_d)[1] == ig.res_rel    # p_dev holds what was measured

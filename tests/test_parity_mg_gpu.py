@@ -208,3 +208,53 @@ def test_diverging_parameters_stop_early(torch_cuda, B):
         info = s.mg_solve(dev(torch_cuda, w.rhs), p_d, 100000, 1e-8)
         assert not info.converged and info.sweeps < 100000
         assert not np.isfinite(info.res_rel)
+
+
+def test_level_memory_is_caller_owned_and_setup_failures_leave_no_half_built_hierarchy(torch_cuda, B, ora):
+    """ps_mg_workspace_bytes / ps_mg_set_workspace: the binding hands the level memory over as a
+    torch allocation; a block that is too small makes ps_mg_setup fail with PS_EINVAL, drops the
+    hierarchy (ps_mg_levels == 0, ps_mg_solve -> PS_ESTATE), and a later set-up with enough memory
+    works and gives the oracle's bits; changing the depth re-uses or rebuilds the chain."""
+    import ctypes
+    w = workload(40, 36, 24, 2, 8, None)
+    prm = dict(levels=2, nu1=1, nu2=1, coarse_sweeps=9, gamma=1, omega_s=1.3, nu_growth=1, nu_max=64)
+    coef = ora.coefficients(w.F, w.rho_l, w.rho_g, w.dx, w.dy, w.dz)
+    p_o = np.zeros_like(w.rhs)
+    ora.mg_solve(coef, w.rhs, p_o, 2, 0.0, **prm)
+    lib = B.load()
+    with B.PoissonSolver(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz) as s:
+        s.set_fraction(dev(torch_cuda, w.F), w.rho_l, w.rho_g)
+        need = lib.ps_mg_workspace_bytes(s._h, 2)
+        assert need > 7 * (w.nx // 2) * (w.ny // 2) * (w.nz // 2) * 8
+        assert lib.ps_mg_workspace_bytes(s._h, 1) == 0
+        deepest = ora.mg_max_levels(w.nx, w.ny, w.nz)             # 3 for this grid
+        assert lib.ps_mg_workspace_bytes(s._h, 99) == lib.ps_mg_workspace_bytes(s._h, deepest) > need
+        small = torch_cuda.empty(need // 2 + 256, dtype=torch_cuda.uint8, device="cuda")
+        base = (small.data_ptr() + 255) // 256 * 256
+        assert lib.ps_mg_set_workspace(s._h, ctypes.c_void_p(base + 8), need) == B.PS_EINVAL   # misaligned
+        assert lib.ps_mg_set_workspace(s._h, ctypes.c_void_p(base), need // 2) == B.PS_OK
+        c_prm = B._MgParams(prm["levels"], prm["nu1"], prm["nu2"], prm["nu_growth"], prm["nu_max"],
+                            prm["coarse_sweeps"], prm["gamma"], prm["omega_s"])
+        assert lib.ps_mg_setup(s._h, ctypes.byref(c_prm)) == B.PS_EINVAL
+        assert lib.ps_mg_levels(s._h) == 0
+        rhs_d = dev(torch_cuda, w.rhs)
+        p_d = torch_cuda.zeros(w.rhs.shape, dtype=torch_cuda.float64, device="cuda")
+        with pytest.raises(B.PsError) as e:
+            s.mg_solve(rhs_d, p_d, 1, 0.0)
+        assert e.value.code == B.PS_ESTATE
+        s._mg_ws = None                       # let the binding allocate a block that fits
+        assert s.mg_setup(**prm) == 2
+        s.mg_solve(rhs_d, p_d, 2, 0.0)
+        same(p_d.cpu().numpy(), p_o, "after a failed set-up")
+        assert s.mg_setup(**dict(prm, levels=1)) == 1             # shallower: chain dropped
+        assert s.mg_setup(**prm) == 2                             # and rebuilt in the same block
+        p_d.zero_()
+        s.mg_solve(rhs_d, p_d, 2, 0.0)
+        same(p_d.cpu().numpy(), p_o, "after a depth change")
+    # library-owned level memory (no torch block): same numbers
+    with B.PoissonSolver(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, workspace=False) as s:
+        s.set_fraction(dev(torch_cuda, w.F), w.rho_l, w.rho_g)
+        assert s.mg_setup(**prm) == 2
+        p_d = torch_cuda.zeros(w.rhs.shape, dtype=torch_cuda.float64, device="cuda")
+        s.mg_solve(dev(torch_cuda, w.rhs), p_d, 2, 0.0)
+        same(p_d.cpu().numpy(), p_o, "library-owned level memory")
