@@ -267,7 +267,7 @@ def run_ours(args, rank):
     if kname != "twopass":
         if args.rpt or args.zchunks:
             s.set_tuning(args.rpt, args.zchunks)
-        tuning = dict(zip(("rows_per_thread", "z_chunks", "tiles"), s.get_tuning()))
+        tuning = dict(zip(("rows_per_thread", "z_chunks", "tiles", "ctas", "items"), s.get_tuning()))
 
     def step():
         p_d.zero_()

@@ -105,13 +105,27 @@ int ps_set_kernel(ps_ctx *c, int variant);
 int ps_get_kernel(const ps_ctx *c);          /* the variant AUTO resolved to, or the one set */
 
 /* Launch geometry of the fused kernel (tuning and tests; every setting gives bitwise identical p).
- * rows_per_thread: rows of the 64x16-cell box one thread updates per step: 1 = 16 compute warps
- * (default, fastest on B200), 2 = 8 compute warps with two rows each, 0 = keep.  z_chunks: number of
- * z chunks each (x,y) tile is cut into (CTAs = tiles * z_chunks), 0 = choose by the cost model
- * (rounds of sm_count CTAs x (planes per chunk + z halo)).  Synchronises the stream.
- * PS_EINVAL: fused kernel not available for this grid, values out of range. */
+ * rows_per_thread: rows of the 64x16-cell box one thread updates per step; only 1 (16 row warps)
+ * is built -- two rows per thread were measured slower on B200 throughout round 1 -- so 0 (keep)
+ * and 1 are accepted.  z_chunks: 0 = the balanced split (the (tile, plane) pairs of the grid cut
+ * into one contiguous range per CTA, every CTA marching the same number of planes); n > 0 = every
+ * (x,y) tile cut into n z chunks, the tile x chunk items dealt round-robin to the CTAs.
+ * Synchronises the stream.  PS_EINVAL: fused kernel not available for this grid, values out of
+ * range.  ps_get_tuning returns the setting, the number of tiles, of CTAs launched and of work
+ * items (any output may be NULL). */
 int ps_set_tuning(ps_ctx *c, int rows_per_thread, int z_chunks);
-int ps_get_tuning(const ps_ctx *c, int *rows_per_thread, int *z_chunks, int *tiles);
+int ps_get_tuning(const ps_ctx *c, int *rows_per_thread, int *z_chunks, int *tiles, int *ctas,
+                  int *items);
+
+/* The work split of the fused kernel as a pure host computation (no device needed; host-logic
+ * tests): tiles of an nx x ny x nz grid and the work items a launch on sm_count SMs would run,
+ * z_chunks as in ps_set_tuning.  tiles_out: 4 ints per tile (xs, xe, ys, ye: owned cells
+ * [xs,xe) x [ys,ye)), at most tile_cap tiles; items_out: 4 ints per item (cta, tile, ks, ke: CTA
+ * `cta` marches tile `tile` over the planes [ks,ke)), in launch order, at most item_cap items;
+ * either may be NULL.  The three counts are always returned.  PS_EINVAL: the fused kernel does
+ * not take this grid (odd nx), bad arguments. */
+int ps_fused_plan(int nx, int ny, int nz, int sm_count, int z_chunks, int *tiles_out, int tile_cap,
+                  int *items_out, int item_cap, int *ntiles, int *nitems, int *nctas);
 
 /* Step 4 of the paper's time step + face coefficients:
  * rho = rho_l F + rho_g (1-F); ax,ay,az = (1/h^2)/(0.5 (rho_c + rho_nb)) for the +x,+y,+z

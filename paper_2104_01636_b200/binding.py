@@ -23,7 +23,7 @@ KERNEL_NAMES = {KERNEL_AUTO: "auto", KERNEL_TWOPASS: "twopass", KERNEL_FUSED: "f
 # every symbol include/ps_poisson.h declares (tests check the library exports each one)
 SYMBOLS = ("ps_create", "ps_destroy", "ps_workspace_bytes", "ps_set_workspace", "ps_set_stream",
            "ps_set_check_interval", "ps_set_kernel", "ps_get_kernel", "ps_set_tuning",
-           "ps_get_tuning", "ps_set_fraction",
+           "ps_get_tuning", "ps_fused_plan", "ps_set_fraction",
            "ps_export_coefficients", "ps_solve", "ps_sweeps", "ps_half_sweep", "ps_residual",
            "ps_solve_host", "ps_host_staging_bytes", "ps_set_host_staging", "ps_enable_timing", "ps_timing", "ps_launch_count", "ps_strerror",
            "ps_mg_workspace_bytes", "ps_mg_set_workspace", "ps_mg_setup", "ps_mg_levels", "ps_mg_solve", "ps_mg_export_coarse",
@@ -84,7 +84,8 @@ def load(path: str | None = None) -> ctypes.CDLL:
     lib.ps_get_kernel.argtypes = [vp]
     lib.ps_set_tuning.argtypes = [vp, i, i]
     ip = ctypes.POINTER(ctypes.c_int)
-    lib.ps_get_tuning.argtypes = [vp, ip, ip, ip]
+    lib.ps_get_tuning.argtypes = [vp, ip, ip, ip, ip, ip]
+    lib.ps_fused_plan.argtypes = [i, i, i, i, i, ip, i, ip, i, ip, ip, ip]
     lib.ps_set_fraction.argtypes = [vp, vp, d, d]
     lib.ps_export_coefficients.argtypes = [vp, vp, vp, vp]
     lib.ps_solve.argtypes = [vp, vp, vp, d, i, d, ctypes.POINTER(_Info)]
@@ -147,6 +148,21 @@ def _host_ptr(a, shape, name):
             and tuple(a.shape) == tuple(shape)):
         raise TypeError(f"{name}: expected a C-contiguous float64 array of shape {tuple(shape)}")
     return ctypes.c_void_p(a.ctypes.data)
+
+
+def fused_plan(nx: int, ny: int, nz: int, sm_count: int = 148, z_chunks: int = 0):
+    """(tiles, items) of the fused kernel's work split (host only): tiles as (xs, xe, ys, ye),
+    items as (cta, tile, ks, ke) in launch order."""
+    lib = load()
+    n = [ctypes.c_int() for _ in range(3)]
+    _check(lib, lib.ps_fused_plan(nx, ny, nz, sm_count, z_chunks, None, 0, None, 0,
+                                  *[ctypes.byref(x) for x in n]))
+    nt, ni = n[0].value, n[1].value
+    tiles, items = (ctypes.c_int * (4 * nt))(), (ctypes.c_int * (4 * ni))()
+    _check(lib, lib.ps_fused_plan(nx, ny, nz, sm_count, z_chunks, tiles, nt, items, ni,
+                                  *[ctypes.byref(x) for x in n]))
+    return ([tuple(tiles[4 * q:4 * q + 4]) for q in range(nt)],
+            [tuple(items[4 * q:4 * q + 4]) for q in range(ni)])
 
 
 class PoissonSolver:
@@ -212,11 +228,10 @@ class PoissonSolver:
         _check(self._lib, self._lib.ps_set_tuning(self._h, rows_per_thread, z_chunks))
 
     def get_tuning(self):
-        """(rows_per_thread, z_chunks, tiles) of the fused kernel's launch geometry."""
-        a, b, c = ctypes.c_int(), ctypes.c_int(), ctypes.c_int()
-        _check(self._lib, self._lib.ps_get_tuning(self._h, ctypes.byref(a), ctypes.byref(b),
-                                                  ctypes.byref(c)))
-        return a.value, b.value, c.value
+        """(rows_per_thread, z_chunks, tiles, ctas, items) of the fused kernel's launch geometry."""
+        v = [ctypes.c_int() for _ in range(5)]
+        _check(self._lib, self._lib.ps_get_tuning(self._h, *[ctypes.byref(x) for x in v]))
+        return tuple(x.value for x in v)
 
     def workspace_bytes(self) -> int:
         return self._lib.ps_workspace_bytes(self._h)

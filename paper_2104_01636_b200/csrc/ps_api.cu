@@ -141,7 +141,7 @@ int resolve_variant(const ps_ctx *c, int req)
         return PS_KERNEL_RESIDENT;
     if (req == PS_KERNEL_AUTO) return fused_ok ? PS_KERNEL_FUSED : PS_KERNEL_TWOPASS;
     if (req == PS_KERNEL_FUSED && !fused_ok) return -1;
-    if (req == PS_KERNEL_FUSED_OTF && !(fused_ok && c->fused.rpt == 1)) return -1;
+    if (req == PS_KERNEL_FUSED_OTF && !fused_ok) return -1;
     if (req == PS_KERNEL_RESIDENT && !c->coop) return -1;
     if (req < PS_KERNEL_AUTO || req > PS_KERNEL_FUSED_OTF) return -1;
     return req;
@@ -390,23 +390,55 @@ int ps_get_kernel(const ps_ctx *c) { return c ? c->variant : PS_EINVAL; }
 int ps_set_tuning(ps_ctx *c, int rows_per_thread, int z_chunks)
 {
     if (!c || !c->fused.ok) return PS_EINVAL;
-    if (rows_per_thread < 0 || rows_per_thread > 2 || z_chunks < 0 || z_chunks > c->g.nz / 2)
+    if (rows_per_thread < 0 || rows_per_thread > 1 || z_chunks < 0 || z_chunks > c->g.nz / 2)
         return PS_EINVAL;
-    const int rpt = rows_per_thread ? rows_per_thread : c->fused.rpt;
-    if (c->variant == PS_KERNEL_FUSED_OTF && rpt != 1) return PS_EINVAL;
     PS_CUDA(cudaStreamSynchronize(c->stream));
-    const cudaError_t e = ps::zm_plan_tiles(&c->fused, c->g, rpt, z_chunks);
+    const cudaError_t e = ps::zm_plan_tiles(&c->fused, c->g, z_chunks);
     if (e == cudaErrorInvalidValue) { cudaGetLastError(); return PS_EINVAL; }
     if (e != cudaSuccess) return cuda_fail(e);
     return PS_OK;
 }
 
-int ps_get_tuning(const ps_ctx *c, int *rows_per_thread, int *z_chunks, int *tiles)
+int ps_get_tuning(const ps_ctx *c, int *rows_per_thread, int *z_chunks, int *tiles, int *ctas,
+                  int *items)
 {
     if (!c || !c->fused.ok) return PS_EINVAL;
-    if (rows_per_thread) *rows_per_thread = c->fused.rpt;
-    if (z_chunks) *z_chunks = c->fused.nchunks;
+    if (rows_per_thread) *rows_per_thread = 1;
+    if (z_chunks) *z_chunks = c->fused.forced ? c->fused.nchunks : 0;
     if (tiles) *tiles = c->fused.ntiles;
+    if (ctas) *ctas = c->fused.ncta;
+    if (items) *items = c->fused.nitems;
+    return PS_OK;
+}
+
+int ps_fused_plan(int nx, int ny, int nz, int sm_count, int z_chunks, int *tiles_out, int tile_cap,
+                  int *items_out, int item_cap, int *ntiles, int *nitems, int *nctas)
+{
+    if (nx < 1 || ny < 1 || nz < 2 || (nz & 1) || sm_count < 1 || z_chunks < 0 || !ntiles ||
+        !nitems || !nctas)
+        return PS_EINVAL;
+    const ps::Grid g{nx, ny, nz};
+    if (!ps::zm_shape_ok(g)) return PS_EINVAL;
+    std::vector<ps::ZmTile> tiles;
+    std::vector<ps::ZmItem> items;
+    std::vector<int> first;
+    int tx = 0, ty = 0, nch = 0, rec = 0;
+    if (!ps::zm_plan_host(g, sm_count, z_chunks, tiles, items, first, &tx, &ty, &nch, &rec))
+        return PS_EINVAL;
+    *ntiles = (int)tiles.size();
+    *nitems = (int)items.size();
+    *nctas = (int)first.size() - 1;
+    if (tiles_out)
+        for (int q = 0; q < *ntiles && q < tile_cap; ++q) {
+            tiles_out[4 * q] = tiles[q].xs; tiles_out[4 * q + 1] = tiles[q].xe;
+            tiles_out[4 * q + 2] = tiles[q].ys; tiles_out[4 * q + 3] = tiles[q].ye;
+        }
+    if (items_out)
+        for (int b = 0; b + 1 < (int)first.size(); ++b)
+            for (int q = first[b]; q < first[b + 1] && q < item_cap; ++q) {
+                items_out[4 * q] = b; items_out[4 * q + 1] = items[q].tile;
+                items_out[4 * q + 2] = items[q].ks; items_out[4 * q + 3] = items[q].ke;
+            }
     return PS_OK;
 }
 

@@ -98,3 +98,50 @@ def test_product_does_not_import_oracle():
                 assert "ps_oracle" not in src and "ora_" not in src, fn
     with open(os.path.join(ROOT, "include", "ps_poisson.h")) as f:
         assert "ps_oracle" not in f.read()
+
+
+@pytest.mark.parametrize("shape", [(256, 256, 512), (128, 128, 256), (384, 384, 1024), (64, 64, 128),
+                                   (32, 32, 64), (186, 46, 8), (130, 44, 4), (2, 2, 2), (66, 17, 6)])
+@pytest.mark.parametrize("z_chunks", [0, 1, 3])
+def test_fused_work_split_covers_every_plane_once_and_is_balanced(lib, shape, z_chunks):
+    """Host logic of the fused kernel's launch (ps_fused_plan, no GPU): the tiles partition the
+    cross-section within the box capacities; the items cover every (tile, plane) exactly once, are
+    grouped per CTA in launch order, have at least 2 planes; and with the automatic split
+    (z_chunks = 0: lockstep rounds of tile x chunk items, the leftover of the last round cut again
+    into one range per CTA) no CTA marches more than a few percent above the mean."""
+    nx, ny, nz = shape
+    if z_chunks > nz // 2:
+        pytest.skip("more chunks than plane pairs")
+    tiles, items = binding.fused_plan(nx, ny, nz, 148, z_chunks)
+    cover = {}
+    for xs, xe, ys, ye in tiles:
+        assert 0 <= xs < xe <= nx and xs % 2 == 0 and xe % 2 == 0 and xe - xs <= 64
+        assert 0 <= ys < ye <= ny
+        rows = (ye - ys) + (ys > 0) + (ye < ny)              # owned rows + red-ring rows
+        assert rows <= 16
+        for i in range(xs, xe, 2):
+            for j in range(ys, ye):
+                assert (i, j) not in cover
+                cover[(i, j)] = 1
+    assert len(cover) == (nx // 2) * ny
+    seen = [[0] * nz for _ in tiles]
+    steps = {}
+    last_cta = -1
+    for cta, tile, ks, ke in items:
+        assert cta in (last_cta, last_cta + 1)               # grouped per CTA, CTAs in order
+        last_cta = cta
+        assert 0 <= ks < ke <= nz and ke - ks >= 2
+        for k in range(ks, ke):
+            seen[tile][k] += 1
+        steps[cta] = steps.get(cta, 0) + (ke - ks) + 3
+    assert all(v == 1 for row in seen for v in row)
+    assert 1 <= len(steps) <= 148
+    if z_chunks == 0:
+        mean = len(tiles) * nz / len(steps)
+        assert max(steps.values()) <= 1.04 * mean + 9, (max(steps.values()), mean)
+
+
+def test_fused_plan_rejects_odd_nx(lib):
+    import ctypes as ct
+    n = [ct.c_int() for _ in range(3)]
+    assert lib.ps_fused_plan(5, 7, 6, 148, 0, None, 0, None, 0, *[ct.byref(x) for x in n]) == binding.PS_EINVAL
