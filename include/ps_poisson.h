@@ -271,6 +271,20 @@ int ps_face_divergence(ps_ctx *c, const double *ux_dev, const double *uy_dev, co
 int ps_ssf_rhs(ps_ctx *c, const double *F_dev, const double *kappa_dev, double sigma,
                double *rhs_dev);
 
+/* Self-checking build (libps_poisson_checked.so, compiled with -DPS_CHECKED; compute-sanitizer is
+ * not available on the B200 pool, profiles/r02_sanitizer.md): the fused sweep kernel checks its
+ * shared-memory addressing, TMA destinations, global stores and its mbarrier ring protocol and
+ * counts violations instead of faulting.  ps_checked_build: 1 in that build, 0 in the product
+ * build.  ps_debug_read: out_host[0] = violations counted since ps_create over this context and
+ * its multigrid levels, out_host[1..5] = the first one (code, three details, CTA << 32 | thread);
+ * all zero in the product build.  Synchronises the stream.
+ * ps_debug_sabotage(c, 1) makes the checked kernel skip the red-barrier wait of its row warps (a
+ * deliberately broken protocol, harmless to memory: the negative control of the checks);
+ * PS_EINVAL in the product build. */
+int ps_checked_build(void);
+int ps_debug_read(ps_ctx *c, unsigned long long *out_host);
+int ps_debug_sabotage(ps_ctx *c, int mode);
+
 /* Kernels launched by this context since ps_create (bench.py's gpu_launches). */
 long long ps_launch_count(const ps_ctx *c);
 

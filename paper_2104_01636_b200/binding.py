@@ -25,7 +25,8 @@ SYMBOLS = ("ps_create", "ps_destroy", "ps_workspace_bytes", "ps_set_workspace", 
            "ps_set_check_interval", "ps_set_kernel", "ps_get_kernel", "ps_set_tuning",
            "ps_get_tuning", "ps_fused_plan", "ps_set_fraction",
            "ps_export_coefficients", "ps_solve", "ps_sweeps", "ps_half_sweep", "ps_residual",
-           "ps_solve_host", "ps_host_staging_bytes", "ps_set_host_staging", "ps_enable_timing", "ps_timing", "ps_launch_count", "ps_strerror",
+           "ps_solve_host", "ps_host_staging_bytes", "ps_set_host_staging", "ps_enable_timing",
+           "ps_checked_build", "ps_debug_read", "ps_debug_sabotage", "ps_timing", "ps_launch_count", "ps_strerror",
            "ps_mg_workspace_bytes", "ps_mg_set_workspace", "ps_mg_setup", "ps_mg_levels", "ps_mg_solve", "ps_mg_export_coarse",
            "ps_mg_residual_restrict", "ps_mg_prolong_add", "ps_rhs_from_velocity",
            "ps_correct_velocity", "ps_face_divergence", "ps_ssf_rhs")
@@ -102,6 +103,9 @@ def load(path: str | None = None) -> ctypes.CDLL:
     lib.ps_mg_workspace_bytes.argtypes = [vp, i]
     lib.ps_mg_workspace_bytes.restype = ctypes.c_size_t
     lib.ps_mg_set_workspace.argtypes = [vp, vp, ctypes.c_size_t]
+    lib.ps_checked_build.argtypes = []
+    lib.ps_debug_read.argtypes = [vp, ctypes.POINTER(ctypes.c_ulonglong)]
+    lib.ps_debug_sabotage.argtypes = [vp, i]
     lib.ps_launch_count.argtypes = [vp]
     lib.ps_launch_count.restype = ctypes.c_longlong
     lib.ps_mg_setup.argtypes = [vp, ctypes.POINTER(_MgParams)]
@@ -169,9 +173,9 @@ class PoissonSolver:
     """ps_create / ps_set_fraction / ps_solve / ps_residual with the names of the C ABI."""
 
     def __init__(self, nx: int, ny: int, nz: int, dx: float, dy: float, dz: float,
-                 workspace: bool = True):
+                 workspace: bool = True, lib=None):
         import torch
-        self._lib = load()
+        self._lib = lib if lib is not None else load()
         self._h = ctypes.c_void_p()
         self.nx, self.ny, self.nz = nx, ny, nz
         self.shape = (nz, ny, nx)
@@ -249,6 +253,12 @@ class PoissonSolver:
 
     def launch_count(self) -> int:
         return self._lib.ps_launch_count(self._h)
+
+    def debug_read(self):
+        """Violation record of the self-checking build (all zero in the product build)."""
+        out = (ctypes.c_ulonglong * 8)()
+        _check(self._lib, self._lib.ps_debug_read(self._h, out))
+        return list(out)
 
     # -- the path
     def set_fraction(self, F, rho_l: float, rho_g: float):

@@ -18,6 +18,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
 _INC = os.path.join(os.path.dirname(_HERE), "include")
 LIB = os.path.join(_HERE, "libps_poisson.so")
+LIB_CHECKED = os.path.join(_HERE, "libps_poisson_checked.so")   # -DPS_CHECKED, tests only
 SOURCES = ["ps_api.cu"]
 HEADERS = sorted(f for f in os.listdir(_CSRC) if f.endswith(".cuh"))
 
@@ -44,16 +45,19 @@ def _deps():
         yield os.path.join(_CSRC, f)
 
 
-def up_to_date() -> bool:
-    return os.path.exists(LIB) and os.path.getmtime(LIB) >= max(os.path.getmtime(d) for d in _deps())
+def up_to_date(lib: str = LIB) -> bool:
+    return os.path.exists(lib) and os.path.getmtime(lib) >= max(os.path.getmtime(d) for d in _deps())
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    """Build libps_poisson.so if missing or older than its sources; returns its path."""
-    if not force and up_to_date():
-        return LIB
-    tmp = f"{LIB}.{os.getpid()}.tmp"
-    cmd = [_nvcc(), *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []),
+def build(force: bool = False, verbose: bool = False, checked: bool = False) -> str:
+    """Build libps_poisson.so (checked: the self-checking libps_poisson_checked.so, compiled with
+    -DPS_CHECKED) if missing or older than its sources; returns its path."""
+    lib = LIB_CHECKED if checked else LIB
+    if not force and up_to_date(lib):
+        return lib
+    tmp = f"{lib}.{os.getpid()}.tmp"
+    cmd = [_nvcc(), *NVCC_FLAGS, *(["-DPS_CHECKED"] if checked else []),
+           *(["-Xptxas", "-v"] if verbose else []),
            "-o", tmp, *[os.path.join(_CSRC, s) for s in SOURCES]]
     res = subprocess.run(cmd, cwd=_CSRC, capture_output=True, text=True)
     if res.returncode != 0:
@@ -62,9 +66,11 @@ def build(force: bool = False, verbose: bool = False) -> str:
         raise RuntimeError("nvcc failed:\n" + " ".join(cmd) + "\n" + res.stdout + res.stderr)
     if verbose:
         sys.stderr.write(res.stdout + res.stderr)
-    os.replace(tmp, LIB)
-    return LIB
+    os.replace(tmp, lib)
+    return lib
 
 
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    if "--checked" in sys.argv:
+        print(build(force="--force" in sys.argv, verbose="-v" in sys.argv, checked=True))

@@ -628,6 +628,45 @@ int ps_timing(ps_ctx *c, double *sweep_ms, long long *sweep_launches, long long 
     return PS_OK;
 }
 
+int ps_checked_build(void)
+{
+#ifdef PS_CHECKED
+    return 1;
+#else
+    return 0;
+#endif
+}
+
+int ps_debug_sabotage(ps_ctx *c, int mode)
+{
+    if (!c || mode < 0 || mode > 1) return PS_EINVAL;
+#ifdef PS_CHECKED
+    c->fused.sabotage = mode;
+    return PS_OK;
+#else
+    return mode == 0 ? PS_OK : PS_EINVAL;           // the product build has no such switch
+#endif
+}
+
+int ps_debug_read(ps_ctx *c, unsigned long long *out_host)
+{
+    if (!c || !out_host) return PS_EINVAL;
+    for (int q = 0; q < 8; ++q) out_host[q] = 0;
+    if (!c->fused.d_dbg) return PS_OK;              // product build / grid without fused kernel
+    PS_CUDA(cudaStreamSynchronize(c->stream));
+    PS_CUDA(cudaMemcpy(out_host, c->fused.d_dbg, 8 * sizeof(unsigned long long),
+                       cudaMemcpyDeviceToHost));
+    for (ps_ctx *k = c->child; k; k = k->child) {   // multigrid levels: add their counts
+        unsigned long long t[8] = {0};
+        if (!k->fused.d_dbg) continue;
+        PS_CUDA(cudaMemcpy(t, k->fused.d_dbg, sizeof t, cudaMemcpyDeviceToHost));
+        if (out_host[0] == 0 && t[0] != 0)
+            for (int q = 1; q < 8; ++q) out_host[q] = t[q];
+        out_host[0] += t[0];
+    }
+    return PS_OK;
+}
+
 long long ps_launch_count(const ps_ctx *c)
 {
     long long n = 0;
