@@ -117,6 +117,21 @@ int ps_set_tuning(ps_ctx *c, int rows_per_thread, int z_chunks);
 int ps_get_tuning(const ps_ctx *c, int *rows_per_thread, int *z_chunks, int *tiles, int *ctas,
                   int *items);
 
+/* Two launch options of the fused kernel (every setting gives bitwise identical p; tests and A/B
+ * measurements switch them, the defaults are what was measured fastest):
+ *   dependent_launch  1 (default): every sweep after the first of a batch is launched with the
+ *                     programmatic stream-serialisation attribute, so its CTAs set up and fetch
+ *                     their first coefficient boxes while the previous sweep drains; 0: plain
+ *                     stream order.
+ *   pace_window       n > 0 (default 2): no CTA issues a stage more than n stages ahead of the
+ *                     mean over all CTAs of the launch, which keeps the halo rows and columns that
+ *                     neighbouring tiles share inside L2 (one global counter, one atomic and one
+ *                     load per CTA and plane); 0: CTAs run free.
+ * -1 keeps a setting.  PS_EINVAL: no fused kernel for this grid, values out of range
+ * (pace_window > 64). */
+int ps_set_launch_options(ps_ctx *c, int dependent_launch, int pace_window);
+int ps_get_launch_options(const ps_ctx *c, int *dependent_launch, int *pace_window);
+
 /* The work split of the fused kernel as a pure host computation (no device needed; host-logic
  * tests): tiles of an nx x ny x nz grid and the work items a launch on sm_count SMs would run,
  * z_chunks as in ps_set_tuning.  tiles_out: 4 ints per tile (xs, xe, ys, ye: owned cells
@@ -192,9 +207,9 @@ int ps_timing(ps_ctx *c, double *sweep_ms, long long *sweep_launches, long long 
  * ny stay even and >= 2 after halving and nz is a multiple of 4; coarse face coefficient =
  * 1/16 of the sum of the 4 fine face coefficients on the coarse face; restriction = mean of the
  * 8 children of r = rhs - A p; piecewise-constant prolongation added to p; red-black SOR
- * (omega_s) as smoother (nu1 before, nu2 after; on level l multiplied by nu_growth^l up to
- * nu_max, because coarse levels are cheap and the bubble modes need them solved accurately)
- * and as coarsest-level solver (coarse_sweeps);
+ * (omega_s on the finest level, omega_c on every coarser one) as smoother (nu1 before, nu2
+ * after; on level l multiplied by nu_growth^l up to nu_max, because coarse levels are cheap and
+ * the bubble modes need them solved accurately) and as coarsest-level solver (coarse_sweeps);
  * gamma = 1 (V cycle) or 2 (W cycle). */
 typedef struct {
     int levels;          /* requested levels, clipped to [1, what the grid allows]            */
@@ -203,7 +218,9 @@ typedef struct {
     int nu_max;          /* cap of the per-level count (>= 1; never lowers nu itself)          */
     int coarse_sweeps;   /* sweeps on the coarsest level (>= 1)                                */
     int gamma;           /* 1 = V, 2 = W                                                       */
-    double omega_s;      /* relaxation factor of smoother and coarsest solver, in (0,2)        */
+    double omega_s;      /* relaxation factor of every sweep on level 0, in (0,2)              */
+    double omega_c;      /* relaxation factor of every sweep on the levels l >= 1 (smoother    */
+                         /* and coarsest solver), in (0,2)                                     */
 } ps_mg_params;
 
 /* Device memory of the coarse levels (per level: coefficients, ping-pong buffer, reduction

@@ -278,7 +278,8 @@ typedef struct {
  * residual, restriction to the rhs of level l+1, zero initial guess there, gamma recursive
  * cycles (1 = V, 2 = W), prolongation added to p, nu2 sweeps.  On level l the smoothing counts are
  * min(nu * nu_growth^l, nu_max) (never below nu): coarse levels are cheap and the bubble modes
- * need them solved accurately (DESIGN.md §12 M6). */
+ * need them solved accurately (DESIGN.md §12 M6).  Every sweep of level 0 uses omega_s, every
+ * sweep of a level l >= 1 (smoothing and the coarsest solve) omega_c. */
 static int mg_nu(int nu, int l, const ora_mg_params *prm)
 {
     long long v = nu;
@@ -289,21 +290,22 @@ static int mg_nu(int nu, int l, const ora_mg_params *prm)
 static void mg_cycle(mg_level *lv, int l, int nlev, const ora_mg_params *prm)
 {
     mg_level *f = &lv[l];
+    const double omega = (l == 0) ? prm->omega_s : prm->omega_c;
     if (l == nlev - 1) {
         for (int s = 0; s < prm->coarse_sweeps; ++s)
-            ora_sweep(f->nx, f->ny, f->nz, f->ax, f->ay, f->az, f->rhs, f->p, prm->omega_s);
+            ora_sweep(f->nx, f->ny, f->nz, f->ax, f->ay, f->az, f->rhs, f->p, omega);
         return;
     }
     mg_level *c = &lv[l + 1];
     for (int s = 0, n1 = mg_nu(prm->nu1, l, prm); s < n1; ++s)
-        ora_sweep(f->nx, f->ny, f->nz, f->ax, f->ay, f->az, f->rhs, f->p, prm->omega_s);
+        ora_sweep(f->nx, f->ny, f->nz, f->ax, f->ay, f->az, f->rhs, f->p, omega);
     ora_mg_residual_field(f->nx, f->ny, f->nz, f->ax, f->ay, f->az, f->rhs, f->p, f->r);
     ora_mg_restrict(f->nx, f->ny, f->nz, f->r, c->rhs);
     memset(c->p, 0, sizeof(double) * (size_t)c->nx * c->ny * c->nz);
     for (int g = 0; g < prm->gamma; ++g) mg_cycle(lv, l + 1, nlev, prm);
     ora_mg_prolong_add(f->nx, f->ny, f->nz, c->p, f->p);
     for (int s = 0, n2 = mg_nu(prm->nu2, l, prm); s < n2; ++s)
-        ora_sweep(f->nx, f->ny, f->nz, f->ax, f->ay, f->az, f->rhs, f->p, prm->omega_s);
+        ora_sweep(f->nx, f->ny, f->nz, f->ax, f->ay, f->az, f->rhs, f->p, omega);
 }
 
 /* Multigrid solve: cycles c = 1..max_cycles from the caller's p, the O5 norm after every cycle,

@@ -39,7 +39,10 @@ typedef struct {
     int nu_max;          /* cap of the per-level smoothing count */
     int coarse_sweeps;   /* SOR sweeps on the coarsest level */
     int gamma;           /* recursive cycles per level: 1 = V, 2 = W */
-    double omega_s;      /* relaxation factor of the smoother and coarsest solver */
+    double omega_s;      /* relaxation factor of the smoother on level 0 (and of the only level when
+                          * levels = 1) */
+    double omega_c;      /* relaxation factor on the coarse levels l >= 1: smoother and coarsest
+                          * solver (DESIGN.md §12 M6) */
 } ora_mg_params;
 
 void ora_mg_coarsen(int nx, int ny, int nz, const double *ax, const double *ay, const double *az,

@@ -23,7 +23,8 @@ KERNEL_NAMES = {KERNEL_AUTO: "auto", KERNEL_TWOPASS: "twopass", KERNEL_FUSED: "f
 # every symbol include/ps_poisson.h declares (tests check the library exports each one)
 SYMBOLS = ("ps_create", "ps_destroy", "ps_workspace_bytes", "ps_set_workspace", "ps_set_stream",
            "ps_set_check_interval", "ps_set_kernel", "ps_get_kernel", "ps_set_tuning",
-           "ps_get_tuning", "ps_fused_plan", "ps_set_fraction",
+           "ps_get_tuning", "ps_set_launch_options", "ps_get_launch_options", "ps_fused_plan",
+           "ps_set_fraction",
            "ps_export_coefficients", "ps_solve", "ps_sweeps", "ps_half_sweep", "ps_residual",
            "ps_solve_host", "ps_host_staging_bytes", "ps_set_host_staging", "ps_enable_timing",
            "ps_checked_build", "ps_debug_read", "ps_debug_sabotage", "ps_timing", "ps_launch_count", "ps_strerror",
@@ -42,7 +43,7 @@ class _MgParams(ctypes.Structure):
     _fields_ = [("levels", ctypes.c_int), ("nu1", ctypes.c_int), ("nu2", ctypes.c_int),
                 ("nu_growth", ctypes.c_int), ("nu_max", ctypes.c_int),
                 ("coarse_sweeps", ctypes.c_int), ("gamma", ctypes.c_int),
-                ("omega_s", ctypes.c_double)]
+                ("omega_s", ctypes.c_double), ("omega_c", ctypes.c_double)]
 
 
 class _Info(ctypes.Structure):
@@ -86,6 +87,8 @@ def load(path: str | None = None) -> ctypes.CDLL:
     lib.ps_set_tuning.argtypes = [vp, i, i]
     ip = ctypes.POINTER(ctypes.c_int)
     lib.ps_get_tuning.argtypes = [vp, ip, ip, ip, ip, ip]
+    lib.ps_set_launch_options.argtypes = [vp, i, i]
+    lib.ps_get_launch_options.argtypes = [vp, ip, ip]
     lib.ps_fused_plan.argtypes = [i, i, i, i, i, ip, i, ip, i, ip, ip, ip]
     lib.ps_set_fraction.argtypes = [vp, vp, d, d]
     lib.ps_export_coefficients.argtypes = [vp, vp, vp, vp]
@@ -237,6 +240,15 @@ class PoissonSolver:
         _check(self._lib, self._lib.ps_get_tuning(self._h, *[ctypes.byref(x) for x in v]))
         return tuple(x.value for x in v)
 
+    def set_launch_options(self, dependent_launch: int = -1, pace_window: int = -1):
+        """Fused kernel: dependent launches (0/1) and the pacing window (0 = off); -1 keeps."""
+        _check(self._lib, self._lib.ps_set_launch_options(self._h, dependent_launch, pace_window))
+
+    def get_launch_options(self):
+        v = [ctypes.c_int() for _ in range(2)]
+        _check(self._lib, self._lib.ps_get_launch_options(self._h, *[ctypes.byref(x) for x in v]))
+        return tuple(x.value for x in v)
+
     def workspace_bytes(self) -> int:
         return self._lib.ps_workspace_bytes(self._h)
 
@@ -304,14 +316,15 @@ class PoissonSolver:
     # -- multigrid acceleration
     def mg_setup(self, levels: int = 6, nu1: int = 0, nu2: int = 2, coarse_sweeps: int = 30,
                  gamma: int = 1, omega_s: float = 1.75, nu_growth: int = 4,
-                 nu_max: int = 16) -> int:
+                 nu_max: int = 16, omega_c: float | None = None) -> int:
         """Build the level hierarchy from the current coefficients; returns the levels in use.
         The defaults are the setting measured fastest to 1e-8 on all five configs
         (profiles/r01_five_configs.md): V(0,2) -- no pre-smoothing, 2 post-smoothing
         sweeps on the finest level, 4x more per coarser level up to 16 --, 30 sweeps on the
         coarsest of 6 levels, omega_s = 1.75 (V(0,2) diverges from omega_s = 1.85 on)."""
         self._sync_stream()
-        prm = _MgParams(levels, nu1, nu2, nu_growth, nu_max, coarse_sweeps, gamma, omega_s)
+        prm = _MgParams(levels, nu1, nu2, nu_growth, nu_max, coarse_sweeps, gamma, omega_s,
+                        omega_s if omega_c is None else omega_c)
         if self._torch_owns:               # the level memory is a torch allocation too
             need = self._lib.ps_mg_workspace_bytes(self._h, levels)
             if need and (self._mg_ws is None or self._mg_ws[0].numel() < need + 256):

@@ -57,6 +57,7 @@ struct ps_ctx {
     bool have_rho;         // rho field of the on-the-fly sweep variant is current
     int sm_count;
     int coop;              // device supports cooperative launches
+    bool pdl;              // fused sweeps after the first of a batch are dependent launches
     long long launches;
     // workspace
     void *ws;
@@ -70,6 +71,10 @@ struct ps_ctx {
     // staging of ps_solve_host: 3 fields, caller-owned (ps_set_host_staging) or cudaMalloc
     double *st_F, *st_rhs, *st_p;
     bool st_owned;
+    // ps_solve_host: second stream for the uploads of rhs and p, which then run beside the
+    // coefficient build; created on first use
+    cudaStream_t copy_stream;
+    cudaEvent_t copy_fork, copy_join;
     ps::ZmPlan fused;
     // optional event timing of the sweep launches (ps_enable_timing)
     bool timing;
@@ -157,6 +162,32 @@ int grid_for(const ps_ctx *c, size_t work_items, int threads)
     return (int)blocks;
 }
 
+// Launch geometry of the z-marching pair stencils (ps_kernels_projection.cuh): tiles of 64 cells x
+// 8 rows, z chunks of *kz planes -- as long as possible (two halo planes of one field per chunk)
+// while the launch still has about two waves of eight blocks per SM.
+dim3 zs_grid(const ps_ctx *c, int wx, int *kz)
+{
+    const int tx = (c->g.nx / 2 + 32 * wx - 1) / (32 * wx), ty = (c->g.ny + 8 / wx - 1) / (8 / wx);
+    const char *ez = getenv("PS_ZS_WAVES");
+    const long long want = (long long)c->sm_count * (ez ? atoi(ez) : 16);
+    long long zc = (want + (long long)tx * ty - 1) / ((long long)tx * ty);
+    const int zc_max = c->g.nz / 8 > 0 ? c->g.nz / 8 : 1;
+    if (zc > zc_max) zc = zc_max;
+    if (zc < 1) zc = 1;
+    *kz = (c->g.nz + (int)zc - 1) / (int)zc;
+    return dim3((unsigned)tx, (unsigned)ty, (unsigned)((c->g.nz + *kz - 1) / *kz));
+}
+
+// warps along x of a block of the z-marching pair stencils: as many as the row fills (a block then
+// reads whole contiguous rows), at most 4
+int zs_wx(const ps_ctx *c)
+{
+    const char *e = getenv("PS_ZS_WX");
+    if (e) return atoi(e) == 4 ? 4 : (atoi(e) == 2 ? 2 : 1);
+    const int pairs = c->g.nx / 2;
+    return pairs > 64 ? 4 : (pairs > 32 ? 2 : 1);
+}
+
 int launch_half_sweep(ps_ctx *c, const double *rhs, double *p, double omega, int colour)
 {
     const size_t items = (size_t)((c->g.nx + 1) / 2) * c->g.ny * c->g.nz;
@@ -229,11 +260,14 @@ int run_sweeps_untimed(ps_ctx *c, const double *rhs, double *p, double **cur, do
     const double c2x = 2.0 * (1.0 / (c->dx * c->dx)), c2y = 2.0 * (1.0 / (c->dy * c->dy)),
                  c2z = 2.0 * (1.0 / (c->dz * c->dz));
     for (int left = n; left > 0; --left) {
+        // every sweep after the first of the batch is a dependent launch: its predecessor in the
+        // stream is a sweep, which writes none of the coefficient, rho or rhs boxes
+        const bool dep = c->pdl && left < n;
         cudaError_t e =
             otf ? ps::zm_launch_otf(c->fused, c->g, c->rho, c2x, c2y, c2z, rhs, src, dst, omega,
-                                    c->stream)
+                                    c->stream, dep)
                 : ps::zm_launch(c->fused, c->g, c->ax, c->ay, c->az, rhs, src, dst, omega,
-                                c->stream);
+                                c->stream, dep);
         c->launches++;
         if (e != cudaSuccess) return cuda_fail(e);
         double *t = src; src = dst; dst = t;
@@ -308,6 +342,7 @@ int ps_create(ps_ctx **out, int nx, int ny, int nz, double dx, double dy, double
     if (!c->ev) { delete c; return PS_ENOMEM; }
     c->dx = dx; c->dy = dy; c->dz = dz;
     c->K = 50;
+    c->pdl = true;
     c->sm_count = sms;
     c->coop = coop;
     c->nparts = nparts_for(c->g.cells());
@@ -336,6 +371,11 @@ int ps_destroy(ps_ctx *c)
     if (c->h_scal) cudaFreeHost(c->h_scal);
     ps::zm_plan_destroy(&c->fused);
     if (c->st_F && c->st_owned) cudaFree(c->st_F);
+    if (c->copy_stream) {
+        cudaStreamDestroy(c->copy_stream);
+        cudaEventDestroy(c->copy_fork);
+        cudaEventDestroy(c->copy_join);
+    }
     if (c->ev) {
         for (cudaEvent_t e : *c->ev) cudaEventDestroy(e);
         delete c->ev;
@@ -408,6 +448,24 @@ int ps_get_tuning(const ps_ctx *c, int *rows_per_thread, int *z_chunks, int *til
     if (tiles) *tiles = c->fused.ntiles;
     if (ctas) *ctas = c->fused.ncta;
     if (items) *items = c->fused.nitems;
+    return PS_OK;
+}
+
+int ps_set_launch_options(ps_ctx *c, int dependent_launch, int pace_window)
+{
+    if (!c || !c->fused.ok) return PS_EINVAL;
+    if (dependent_launch < -1 || dependent_launch > 1 || pace_window < -1 || pace_window > 64)
+        return PS_EINVAL;
+    if (dependent_launch >= 0) c->pdl = dependent_launch != 0;
+    if (pace_window >= 0) c->fused.pace_window = pace_window;
+    return PS_OK;
+}
+
+int ps_get_launch_options(const ps_ctx *c, int *dependent_launch, int *pace_window)
+{
+    if (!c || !c->fused.ok) return PS_EINVAL;
+    if (dependent_launch) *dependent_launch = c->pdl ? 1 : 0;
+    if (pace_window) *pace_window = c->fused.pace_window;
     return PS_OK;
 }
 
@@ -590,11 +648,22 @@ int ps_solve_host(ps_ctx *c, const double *F_host, double rho_l, double rho_g,
         ps_set_host_staging(c, st, 3 * field_bytes(c));
         c->st_owned = true;
     }
+    if (!c->copy_stream) {
+        PS_CUDA(cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+        PS_CUDA(cudaEventCreateWithFlags(&c->copy_fork, cudaEventDisableTiming));
+        PS_CUDA(cudaEventCreateWithFlags(&c->copy_join, cudaEventDisableTiming));
+    }
+    // F first; rhs and p follow on the copy stream (ordered after F and after everything already
+    // queued on the context's stream), so the coefficient build runs beside their upload
     PS_CUDA(cudaMemcpyAsync(c->st_F, F_host, b, cudaMemcpyHostToDevice, c->stream));
+    PS_CUDA(cudaEventRecord(c->copy_fork, c->stream));
+    PS_CUDA(cudaStreamWaitEvent(c->copy_stream, c->copy_fork, 0));
+    PS_CUDA(cudaMemcpyAsync(c->st_rhs, rhs_host, b, cudaMemcpyHostToDevice, c->copy_stream));
+    PS_CUDA(cudaMemcpyAsync(c->st_p, p_host, b, cudaMemcpyHostToDevice, c->copy_stream));
+    PS_CUDA(cudaEventRecord(c->copy_join, c->copy_stream));
     int rc = ps_set_fraction(c, c->st_F, rho_l, rho_g);
+    PS_CUDA(cudaStreamWaitEvent(c->stream, c->copy_join, 0));
     if (rc) return rc;
-    PS_CUDA(cudaMemcpyAsync(c->st_rhs, rhs_host, b, cudaMemcpyHostToDevice, c->stream));
-    PS_CUDA(cudaMemcpyAsync(c->st_p, p_host, b, cudaMemcpyHostToDevice, c->stream));
     rc = ps_solve(c, c->st_rhs, c->st_p, omega, max_sweeps, tol, info);
     if (rc) return rc;
     PS_CUDA(cudaMemcpyAsync(p_host, c->st_p, b, cudaMemcpyDeviceToHost, c->stream));
@@ -746,11 +815,6 @@ int mg_build_levels(ps_ctx *c, int nlev)
 
 int mg_launch_coarsen(ps_ctx *f, ps_ctx *k)
 {
-    const char *exp_ = getenv("PS_EXP_COARSEN");
-    if (exp_ && exp_[0] == '1')
-        ps::ps_mg_coarsen_series_kernel<<<grid_for(f, k->g.cells(), 256), 256, 0, f->stream>>>(
-            f->g, f->ax, f->ay, f->az, k->ax, k->ay, k->az);
-    else
     ps::ps_mg_coarsen_kernel<<<grid_for(f, k->g.cells(), 256), 256, 0, f->stream>>>(
         f->g, f->ax, f->ay, f->az, k->ax, k->ay, k->az);
     f->launches++;
@@ -814,18 +878,19 @@ int mg_cycle(ps_ctx *f, const ps_mg_params &m, const double *rhs, double *p, int
              bool restricted = false)
 {
     int rc;
+    const double omega = level == 0 ? m.omega_s : m.omega_c;
     if (!f->child || f->mg_nlev <= 1)
-        return run_sweeps_inplace(f, rhs, p, m.omega_s, m.coarse_sweeps);
+        return run_sweeps_inplace(f, rhs, p, omega, m.coarse_sweeps);
     ps_ctx *k = f->child;
     if (!restricted) {
-        if ((rc = run_sweeps_inplace(f, rhs, p, m.omega_s, mg_nu(m.nu1, level, m)))) return rc;
+        if ((rc = run_sweeps_inplace(f, rhs, p, omega, mg_nu(m.nu1, level, m)))) return rc;
         if ((rc = mg_launch_residual_restrict(f, rhs, p, k->lv_rhs))) return rc;
     }
     PS_CUDA(cudaMemsetAsync(k->lv_p, 0, k->g.cells() * sizeof(double), f->stream));
     for (int g = 0; g < m.gamma; ++g)
         if ((rc = mg_cycle(k, m, k->lv_rhs, k->lv_p, level + 1))) return rc;
     if ((rc = mg_launch_prolong_add(f, k->lv_p, p))) return rc;
-    return run_sweeps_inplace(f, rhs, p, m.omega_s, mg_nu(m.nu2, level, m));
+    return run_sweeps_inplace(f, rhs, p, omega, mg_nu(m.nu2, level, m));
 }
 
 }  // namespace
@@ -856,7 +921,8 @@ int ps_mg_setup(ps_ctx *c, const ps_mg_params *prm)
     if (!c || !prm) return PS_EINVAL;
     if (prm->nu1 < 0 || prm->nu2 < 0 || prm->nu_growth < 1 || prm->nu_max < 1 ||
         prm->coarse_sweeps < 1 || prm->gamma < 1 ||
-        prm->gamma > 2 || !(prm->omega_s > 0.0 && prm->omega_s < 2.0))
+        prm->gamma > 2 || !(prm->omega_s > 0.0 && prm->omega_s < 2.0) ||
+        !(prm->omega_c > 0.0 && prm->omega_c < 2.0))
         return PS_EINVAL;
     if (!c->have_coef) return PS_ESTATE;
     int dev = -1;
@@ -977,11 +1043,20 @@ int ps_rhs_from_velocity(ps_ctx *c, const double *ux_dev, const double *uy_dev,
     if (!(dt > 0.0) || !std::isfinite(dt)) return PS_EINVAL;
     if (!aligned16(ux_dev, uy_dev, uz_dev, rhs_dev)) return PS_EINVAL;
     const ps::Spacing h{c->dx, c->dy, c->dz};
-    if (c->g.nx % 2 == 0)
-        ps::ps_rhs_from_velocity_pair_kernel<<<grid_for(c, c->g.cells() / 2, 256), 256, 0,
-                                               c->stream>>>(c->g, h, ux_dev, uy_dev, uz_dev, dt,
-                                                            rhs_dev);
-    else
+    int kz = 0;
+    const int wx = zs_wx(c);
+    if (c->g.nx % 2 == 0 && c->g.ny <= 65535) {
+        const dim3 grid = zs_grid(c, wx, &kz);
+        if (wx == 4)
+            ps::ps_rhs_from_velocity_pair_kernel<4><<<grid, ps::ZS_THREADS, 0, c->stream>>>(
+                c->g, h, ux_dev, uy_dev, uz_dev, dt, rhs_dev, kz);
+        else if (wx == 2)
+            ps::ps_rhs_from_velocity_pair_kernel<2><<<grid, ps::ZS_THREADS, 0, c->stream>>>(
+                c->g, h, ux_dev, uy_dev, uz_dev, dt, rhs_dev, kz);
+        else
+            ps::ps_rhs_from_velocity_pair_kernel<1><<<grid, ps::ZS_THREADS, 0, c->stream>>>(
+                c->g, h, ux_dev, uy_dev, uz_dev, dt, rhs_dev, kz);
+    } else
         ps::ps_rhs_from_velocity_kernel<<<grid_for(c, c->g.cells(), 256), 256, 0, c->stream>>>(
             c->g, h, ux_dev, uy_dev, uz_dev, dt, rhs_dev);
     c->launches++;
@@ -1012,11 +1087,20 @@ int ps_face_divergence(ps_ctx *c, const double *ux_dev, const double *uy_dev, co
     if (!aligned16(ux_dev, uy_dev, uz_dev, p_dev) || !aligned16(div_dev)) return PS_EINVAL;
     if (!c->have_coef) return PS_ESTATE;
     const ps::Spacing h{c->dx, c->dy, c->dz};
-    if (c->g.nx % 2 == 0)
-        ps::ps_face_divergence_pair_kernel<<<grid_for(c, c->g.cells() / 2, 256), 256, 0,
-                                             c->stream>>>(c->g, h, c->ax, c->ay, c->az, ux_dev,
-                                                          uy_dev, uz_dev, p_dev, dt, div_dev);
-    else
+    int kz = 0;
+    const int wx = zs_wx(c);
+    if (c->g.nx % 2 == 0 && c->g.ny <= 65535) {
+        const dim3 grid = zs_grid(c, wx, &kz);
+        if (wx == 4)
+            ps::ps_face_divergence_pair_kernel<4><<<grid, ps::ZS_THREADS, 0, c->stream>>>(
+                c->g, h, c->ax, c->ay, c->az, ux_dev, uy_dev, uz_dev, p_dev, dt, div_dev, kz);
+        else if (wx == 2)
+            ps::ps_face_divergence_pair_kernel<2><<<grid, ps::ZS_THREADS, 0, c->stream>>>(
+                c->g, h, c->ax, c->ay, c->az, ux_dev, uy_dev, uz_dev, p_dev, dt, div_dev, kz);
+        else
+            ps::ps_face_divergence_pair_kernel<1><<<grid, ps::ZS_THREADS, 0, c->stream>>>(
+                c->g, h, c->ax, c->ay, c->az, ux_dev, uy_dev, uz_dev, p_dev, dt, div_dev, kz);
+    } else
         ps::ps_face_divergence_kernel<<<grid_for(c, c->g.cells(), 256), 256, 0, c->stream>>>(
             c->g, h, c->ax, c->ay, c->az, ux_dev, uy_dev, uz_dev, p_dev, dt, div_dev);
     c->launches++;

@@ -35,45 +35,6 @@ ps_mg_coarsen_kernel(Grid gf, const double *__restrict__ ax, const double *__res
     }
 }
 
-// EXPERIMENT (series/parallel homogenisation): coarse face = 1/8 sum over the 4 strands of
-// 1 / (0.5/a0 + 1/a1 + 0.5/a2), a0, a1, a2 the three fine faces between the centres of the two
-// coarse cells along the face normal.
-__device__ __forceinline__ double mg_series(double a0, double a1, double a2)
-{
-    return 1.0 / (((0.5 / a0) + (1.0 / a1)) + (0.5 / a2));
-}
-
-__global__ void __launch_bounds__(256)
-ps_mg_coarsen_series_kernel(Grid gf, const double *__restrict__ ax, const double *__restrict__ ay,
-                            const double *__restrict__ az, double *__restrict__ axc,
-                            double *__restrict__ ayc, double *__restrict__ azc)
-{
-    const int cx = gf.nx >> 1, cy = gf.ny >> 1, cz = gf.nz >> 1;
-    const size_t NC = (size_t)cx * cy * cz;
-    const size_t sx = 1, sy = (size_t)gf.nx, sz = (size_t)gf.nx * gf.ny;
-    for (size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x; c < NC;
-         c += (size_t)gridDim.x * blockDim.x) {
-        const int I = (int)((unsigned)c % (unsigned)cx);
-        const unsigned t = (unsigned)c / (unsigned)cx;
-        const int J = (int)(t % (unsigned)cy), K = (int)(t / (unsigned)cy);
-        const size_t n = gf.idx(2 * I, 2 * J, 2 * K);
-        const size_t zup = (2 * K + 2 < gf.nz) ? 2 * sz : (size_t)0 - (size_t)(gf.nz - 2) * sz;
-        double vx = 0.0, vy = 0.0, vz = 0.0;
-#pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            const size_t ox = n + (q & 1) * sy + (q >> 1) * sz;
-            const size_t oy = n + (q & 1) * sx + (q >> 1) * sz;
-            const size_t oz = n + (q & 1) * sx + (q >> 1) * sy;
-            if (I + 1 < cx) vx = vx + mg_series(ax[ox], ax[ox + sx], ax[ox + 2 * sx]);
-            if (J + 1 < cy) vy = vy + mg_series(ay[oy], ay[oy + sy], ay[oy + 2 * sy]);
-            vz = vz + mg_series(az[oz], az[oz + sz], az[oz + zup]);
-        }
-        axc[c] = 0.125 * vx;
-        ayc[c] = 0.125 * vy;
-        azc[c] = 0.125 * vz;
-    }
-}
-
 // M2 + M3 fused: the residual of the 8 children (4 x-pairs, 16-byte loads), summed with x fastest,
 // then y, then z, times 1/8.  The residual field itself is never stored (saves 16 B per fine cell
 // of traffic).  nx is even on every level that is coarsened.

@@ -198,3 +198,46 @@ def test_level_dependent_smoothing_counts(ora):
     ora.mg_prolong_add(e1, q)
     ora.sweep(coef, rhs, q, 1.3, 1)
     assert np.array_equal(p, q)
+
+
+def test_coarse_levels_relax_with_omega_c(ora):
+    """M6: omega_s relaxes level 0 only, omega_c every level below it (smoothing and the coarsest
+    solve) -- a 3-level V(1,2) cycle against hand-unrolled oracle steps with two different
+    factors; omega_c = None is the one-factor cycle; one level never sees omega_c."""
+    nx, ny, nz = 8, 8, 16
+    coef = var_coef(ora, nx, ny, nz, 51)
+    rhs = wl.remove_mean(rnd((nz, ny, nx), 52))
+    w0, wc = 1.15, 1.85
+    p = np.zeros_like(rhs)
+    ora.mg_solve(coef, rhs, p, 1, 0.0, levels=3, nu1=1, nu2=2, coarse_sweeps=5, omega_s=w0,
+                 omega_c=wc, nu_growth=2, nu_max=100)
+    c1 = ora.mg_coarsen(coef)
+    c2 = ora.mg_coarsen(c1)
+    q = np.zeros_like(rhs)
+    ora.sweep(coef, rhs, q, w0, 1)
+    r1 = ora.mg_restrict(ora.mg_residual_field(coef, rhs, q))
+    e1 = np.zeros_like(r1)
+    ora.sweep(c1, r1, e1, wc, 2)
+    r2 = ora.mg_restrict(ora.mg_residual_field(c1, r1, e1))
+    e2 = np.zeros_like(r2)
+    ora.sweep(c2, r2, e2, wc, 5)
+    ora.mg_prolong_add(e2, e1)
+    ora.sweep(c1, r1, e1, wc, 4)
+    ora.mg_prolong_add(e1, q)
+    ora.sweep(coef, rhs, q, w0, 2)
+    assert np.array_equal(p, q)
+    # swapping the two factors is a different iteration (the pin would not see a cycle that
+    # ignored omega_c or used it on level 0)
+    s = np.zeros_like(rhs)
+    ora.mg_solve(coef, rhs, s, 1, 0.0, levels=3, nu1=1, nu2=2, coarse_sweeps=5, omega_s=wc,
+                 omega_c=w0, nu_growth=2, nu_max=100)
+    assert not np.array_equal(s, p)
+    a, b = np.zeros_like(rhs), np.zeros_like(rhs)
+    ora.mg_solve(coef, rhs, a, 2, 0.0, levels=3, nu1=1, nu2=1, coarse_sweeps=5, omega_s=1.3)
+    ora.mg_solve(coef, rhs, b, 2, 0.0, levels=3, nu1=1, nu2=1, coarse_sweeps=5, omega_s=1.3,
+                 omega_c=1.3)
+    assert np.array_equal(a, b)
+    a, b = np.zeros_like(rhs), np.zeros_like(rhs)
+    ora.mg_solve(coef, rhs, a, 1, 0.0, levels=1, coarse_sweeps=7, omega_s=1.3, omega_c=0.7)
+    ora.sweep(coef, rhs, b, 1.3, 7)
+    assert np.array_equal(a, b)

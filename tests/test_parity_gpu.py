@@ -42,10 +42,12 @@ def assert_p_parity(p_gpu, p_ora, what=""):
     assert nbad == 0, f"{what}: {nbad} doubles differ (max-rel {diff:.3e})"
 
 
-def variants_for(B, w, tunings=((1, 0), (1, 1), (1, 2), (1, 3))):
+def variants_for(B, w, tunings=((1, 0, -1, -1), (1, 1, 0, 0), (1, 2, 1, 0), (1, 3, 0, 4),
+                                 (1, 0, 1, 1))):
     """Kernel variants the library accepts for this grid shape (asked of the library itself):
-    (kernel, rows_per_thread, z_chunks); the fused kernel is run in several launch geometries
-    (z_chunks = 0: the balanced split bench.py times; n > 0: tile x chunk items)."""
+    (kernel, rows_per_thread, z_chunks, dependent_launch, pace_window); the fused kernel is run
+    in several launch geometries (z_chunks = 0: the balanced split bench.py times; n > 0: tile x
+    chunk items) and with its launch options on and off (-1: the library defaults)."""
     out = []
     with B.PoissonSolver(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, workspace=False) as s:
         for v in (B.KERNEL_TWOPASS, B.KERNEL_RESIDENT, B.KERNEL_FUSED_OTF, B.KERNEL_FUSED):
@@ -54,12 +56,13 @@ def variants_for(B, w, tunings=((1, 0), (1, 1), (1, 2), (1, 3))):
             except B.PsError:
                 continue
             if v in (B.KERNEL_TWOPASS, B.KERNEL_RESIDENT):
-                out.append((v, 0, 0))
+                out.append((v, 0, 0, -1, -1))
                 continue
-            for rpt, chunks in tunings:
+            for rpt, chunks, dep, window in tunings:
                 try:
                     s.set_tuning(rpt, chunks)
-                    out.append((v, rpt, chunks))
+                    s.set_launch_options(dep, window)
+                    out.append((v, rpt, chunks, dep, window))
                 except B.PsError:
                     pass
     return out
@@ -68,10 +71,11 @@ def variants_for(B, w, tunings=((1, 0), (1, 1), (1, 2), (1, 3))):
 def make_solver(B, w, variant=None):
     s = B.PoissonSolver(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz)
     if variant is not None:
-        kernel, rpt, chunks = variant
+        kernel, rpt, chunks, dep, window = variant
         s.set_kernel(kernel)
         if kernel not in (B.KERNEL_TWOPASS, B.KERNEL_RESIDENT):
             s.set_tuning(rpt, chunks)
+            s.set_launch_options(dep, window)
     return s
 
 
@@ -467,24 +471,28 @@ def test_subnormal_coefficients_bitwise(torch_cuda, B, ora):
 
 def test_long_run_repeatable_across_fused_variants(torch_cuda, B):
     """2,000 sweeps on config 3 (18 tiles, every SM busy): the fused kernel twice with the balanced
-    split, with 5 and with 9 z chunks per tile, and the on-the-fly variant all end on the same
-    bits -- a rare miss in the mbarrier protocol (a stage read before it landed, a red value read
+    split, without dependent launches and pacing, with 5 and with 9 z chunks per tile under other
+    pacing windows, and the on-the-fly variant all end on the same bits -- a rare miss in the mbarrier protocol (a stage read before it landed, a red value read
     before it was written) would show up as a difference between runs."""
     w = wl.make_config(3)
     F_d, rhs_d = to_dev(torch_cuda, w.F), to_dev(torch_cuda, w.rhs)
     ref = None
-    for kernel, rpt, chunks in [(B.KERNEL_FUSED, 1, 0), (B.KERNEL_FUSED, 1, 0), (B.KERNEL_FUSED, 1, 5),
-                                (B.KERNEL_FUSED, 1, 9), (B.KERNEL_FUSED_OTF, 1, 0)]:
+    # (kernel, rows per thread, z chunks, dependent launches, pacing window; -1 = library default)
+    for kernel, rpt, chunks, dep, window in [
+            (B.KERNEL_FUSED, 1, 0, -1, -1), (B.KERNEL_FUSED, 1, 0, -1, -1),
+            (B.KERNEL_FUSED, 1, 0, 0, 0), (B.KERNEL_FUSED, 1, 5, 1, 1), (B.KERNEL_FUSED, 1, 9, 0, 8),
+            (B.KERNEL_FUSED_OTF, 1, 0, -1, -1)]:
         with B.PoissonSolver(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz) as s:
             s.set_kernel(kernel)
             s.set_tuning(rpt, chunks)
+            s.set_launch_options(dep, window)
             s.set_fraction(F_d, w.rho_l, w.rho_g)
             p_d = torch_cuda.zeros_like(rhs_d)
             s.sweeps(rhs_d, p_d, w.omega, 2000)
             if ref is None:
                 ref = p_d.clone()
             else:
-                assert torch_cuda.equal(p_d, ref), (kernel, rpt, chunks)
+                assert torch_cuda.equal(p_d, ref), (kernel, rpt, chunks, dep, window)
 
 
 def test_unaligned_pointers_are_rejected_everywhere(torch_cuda, B, ora):

@@ -234,7 +234,7 @@ def test_level_memory_is_caller_owned_and_setup_failures_leave_no_half_built_hie
         assert lib.ps_mg_set_workspace(s._h, ctypes.c_void_p(base + 8), need) == B.PS_EINVAL   # misaligned
         assert lib.ps_mg_set_workspace(s._h, ctypes.c_void_p(base), need // 2) == B.PS_OK
         c_prm = B._MgParams(prm["levels"], prm["nu1"], prm["nu2"], prm["nu_growth"], prm["nu_max"],
-                            prm["coarse_sweeps"], prm["gamma"], prm["omega_s"])
+                            prm["coarse_sweeps"], prm["gamma"], prm["omega_s"], prm["omega_s"])
         assert lib.ps_mg_setup(s._h, ctypes.byref(c_prm)) == B.PS_EINVAL
         assert lib.ps_mg_levels(s._h) == 0
         rhs_d = dev(torch_cuda, w.rhs)
