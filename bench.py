@@ -58,7 +58,7 @@ PLAIN_SOR_RECORDED = {
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json config 1..5 (default 4)")
@@ -71,6 +71,10 @@ def parse_args():
                          "8M cells, 20000 beyond; 0 = skip)")
     ap.add_argument("--rpt", type=int, default=0, help="fused kernel: rows per thread (0 = auto)")
     ap.add_argument("--zchunks", type=int, default=0, help="fused kernel: z chunks (0 = auto)")
+    ap.add_argument("--pace-window", type=int, default=-1,
+                    help="fused kernel: pacing window (0 = off, -1 = library default)")
+    ap.add_argument("--dependent-launch", type=int, default=-1,
+                    help="fused kernel: dependent launches 0/1 (-1 = library default)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="oracle sample budget")
@@ -268,6 +272,8 @@ def run_ours(args, rank):
         if args.rpt or args.zchunks:
             s.set_tuning(args.rpt, args.zchunks)
         tuning = dict(zip(("rows_per_thread", "z_chunks", "tiles", "ctas", "items"), s.get_tuning()))
+        s.set_launch_options(args.dependent_launch, args.pace_window)
+        tuning.update(zip(("dependent_launch", "pace_window"), s.get_launch_options()))
 
     def step():
         p_d.zero_()

@@ -20,6 +20,15 @@ KERNEL_AUTO, KERNEL_TWOPASS, KERNEL_FUSED, KERNEL_RESIDENT, KERNEL_FUSED_OTF = 0
 KERNEL_NAMES = {KERNEL_AUTO: "auto", KERNEL_TWOPASS: "twopass", KERNEL_FUSED: "fused",
                 KERNEL_RESIDENT: "resident", KERNEL_FUSED_OTF: "fused_otf"}
 
+# Multigrid parameters `mg_setup()` uses when none are given (measured fastest to
+# 1e-8 on the bubbly configs among ~500 settings, profiles/r02_mg_tuning.md): V(0,2) -- no
+# pre-smoothing, 2 post-smoothing sweeps on the finest level at omega_s = 1.5 --, 32 sweeps at
+# omega_c = 1.95 on every coarser level, 10 on the coarsest of 6.  omega_c = 1.97 still converges on
+# every config, 1.98 does not.  The one place they are written down: bench.py, report.py and the
+# parity tests take them from here.
+MG_DEFAULTS = dict(levels=6, nu1=0, nu2=2, coarse_sweeps=10, gamma=1, omega_s=1.5, omega_c=1.95,
+                   nu_growth=16, nu_max=32)
+
 # every symbol include/ps_poisson.h declares (tests check the library exports each one)
 SYMBOLS = ("ps_create", "ps_destroy", "ps_workspace_bytes", "ps_set_workspace", "ps_set_stream",
            "ps_set_check_interval", "ps_set_kernel", "ps_get_kernel", "ps_set_tuning",
@@ -241,7 +250,8 @@ class PoissonSolver:
         return tuple(x.value for x in v)
 
     def set_launch_options(self, dependent_launch: int = -1, pace_window: int = -1):
-        """Fused kernel: dependent launches (0/1) and the pacing window (0 = off); -1 keeps."""
+        """Fused kernel: dependent launches (0/1) and the pacing window (0 = off); -1 leaves the
+        choice to the library."""
         _check(self._lib, self._lib.ps_set_launch_options(self._h, dependent_launch, pace_window))
 
     def get_launch_options(self):
@@ -314,17 +324,24 @@ class PoissonSolver:
         return ra.value, rr.value, bn.value
 
     # -- multigrid acceleration
-    def mg_setup(self, levels: int = 6, nu1: int = 0, nu2: int = 2, coarse_sweeps: int = 30,
-                 gamma: int = 1, omega_s: float = 1.75, nu_growth: int = 4,
-                 nu_max: int = 16, omega_c: float | None = None) -> int:
+    def mg_setup(self, levels: int | None = None, nu1: int | None = None, nu2: int | None = None,
+                 coarse_sweeps: int | None = None, gamma: int | None = None,
+                 omega_s: float | None = None, nu_growth: int | None = None,
+                 nu_max: int | None = None, omega_c: float | None = None) -> int:
         """Build the level hierarchy from the current coefficients; returns the levels in use.
-        The defaults are the setting measured fastest to 1e-8 on all five configs
-        (profiles/r01_five_configs.md): V(0,2) -- no pre-smoothing, 2 post-smoothing
-        sweeps on the finest level, 4x more per coarser level up to 16 --, 30 sweeps on the
-        coarsest of 6 levels, omega_s = 1.75 (V(0,2) diverges from omega_s = 1.85 on)."""
+        With no arguments: MG_DEFAULTS.  Any argument given replaces its default, except that
+        omega_c follows an explicitly given omega_s when it is not given itself (one relaxation
+        factor on every level)."""
         self._sync_stream()
-        prm = _MgParams(levels, nu1, nu2, nu_growth, nu_max, coarse_sweeps, gamma, omega_s,
-                        omega_s if omega_c is None else omega_c)
+        if omega_c is None and omega_s is not None:
+            omega_c = omega_s
+        given = dict(levels=levels, nu1=nu1, nu2=nu2, coarse_sweeps=coarse_sweeps, gamma=gamma,
+                     omega_s=omega_s, omega_c=omega_c, nu_growth=nu_growth, nu_max=nu_max)
+        q = dict(MG_DEFAULTS)
+        q.update({k: v for k, v in given.items() if v is not None})
+        levels = q["levels"]
+        prm = _MgParams(q["levels"], q["nu1"], q["nu2"], q["nu_growth"], q["nu_max"],
+                        q["coarse_sweeps"], q["gamma"], q["omega_s"], q["omega_c"])
         if self._torch_owns:               # the level memory is a torch allocation too
             need = self._lib.ps_mg_workspace_bytes(self._h, levels)
             if need and (self._mg_ws is None or self._mg_ws[0].numel() < need + 256):

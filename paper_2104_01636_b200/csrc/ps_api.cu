@@ -57,7 +57,8 @@ struct ps_ctx {
     bool have_rho;         // rho field of the on-the-fly sweep variant is current
     int sm_count;
     int coop;              // device supports cooperative launches
-    bool pdl;              // fused sweeps after the first of a batch are dependent launches
+    int pdl_mode;          // dependent launches of the fused sweeps: -1 automatic, 0 off, 1 on
+    int pace_mode;         // pacing window of the fused sweeps: -1 automatic, 0 off, n
     long long launches;
     // workspace
     void *ws;
@@ -137,6 +138,27 @@ int ensure_workspace(ps_ctx *c)
     return PS_OK;
 }
 
+// Launch options of the fused sweep when the caller leaves them to the library (measured on one
+// B200 in sustained, power-capped runs of bench.py and in cold bursts; DESIGN.md 7.1,
+// profiles/r02_launch_options.md):
+//  * dependent launches pay where a launch is short (config 2, 8 steps per CTA: 10.2 -> 6.9 us per
+//    sweep; config 3, 35 steps: 37.0 -> 35.3) and cost 4 % in sustained runs of long launches
+//    (config 4, 270 steps: 129.1 -> 124.0 Gcell-updates/s at the power cap);
+//  * pacing cuts the DRAM traffic of cold bursts at full clocks (config 5: 1.19 -> 1.06 x
+//    algorithmic, 112 -> 137 Gcell-updates/s) but costs 8 % in sustained runs on every config
+//    (config 5: 131.3 -> 120.4), the regime a solver lives in: off unless asked for.
+constexpr int ps_pdl_max_steps = 96;      // dependent launches up to this many steps per CTA
+
+bool launch_dependent(const ps_ctx *c)
+{
+    return c->pdl_mode < 0 ? c->fused.pace_steps <= ps_pdl_max_steps : c->pdl_mode != 0;
+}
+
+int launch_pace_window(const ps_ctx *c)
+{
+    return c->pace_mode >= 0 ? c->pace_mode : 0;
+}
+
 int resolve_variant(const ps_ctx *c, int req)
 {
     const bool fused_ok = c->fused.ok;
@@ -163,29 +185,19 @@ int grid_for(const ps_ctx *c, size_t work_items, int threads)
 }
 
 // Launch geometry of the z-marching pair stencils (ps_kernels_projection.cuh): tiles of 64 cells x
-// 8 rows, z chunks of *kz planes -- as long as possible (two halo planes of one field per chunk)
-// while the launch still has about two waves of eight blocks per SM.
-dim3 zs_grid(const ps_ctx *c, int wx, int *kz)
+// 8 rows, z chunks of *kz planes (two halo planes of one field per chunk), about `waves` blocks
+// per SM in the launch.  Measured on config 4: ps_rhs_from_velocity 225 / 212 / 197 us with 8 /
+// 16 / 32 blocks per SM, ps_face_divergence 376 / 388 / 382 us.
+dim3 zs_grid(const ps_ctx *c, int waves, int *kz)
 {
-    const int tx = (c->g.nx / 2 + 32 * wx - 1) / (32 * wx), ty = (c->g.ny + 8 / wx - 1) / (8 / wx);
-    const char *ez = getenv("PS_ZS_WAVES");
-    const long long want = (long long)c->sm_count * (ez ? atoi(ez) : 16);
+    const int tx = (c->g.nx / 2 + ps::ZS_TX - 1) / ps::ZS_TX, ty = (c->g.ny + ps::ZS_TY - 1) / ps::ZS_TY;
+    const long long want = (long long)c->sm_count * waves;
     long long zc = (want + (long long)tx * ty - 1) / ((long long)tx * ty);
-    const int zc_max = c->g.nz / 8 > 0 ? c->g.nz / 8 : 1;
+    const int zc_max = c->g.nz / 4 > 0 ? c->g.nz / 4 : 1;
     if (zc > zc_max) zc = zc_max;
     if (zc < 1) zc = 1;
     *kz = (c->g.nz + (int)zc - 1) / (int)zc;
     return dim3((unsigned)tx, (unsigned)ty, (unsigned)((c->g.nz + *kz - 1) / *kz));
-}
-
-// warps along x of a block of the z-marching pair stencils: as many as the row fills (a block then
-// reads whole contiguous rows), at most 4
-int zs_wx(const ps_ctx *c)
-{
-    const char *e = getenv("PS_ZS_WX");
-    if (e) return atoi(e) == 4 ? 4 : (atoi(e) == 2 ? 2 : 1);
-    const int pairs = c->g.nx / 2;
-    return pairs > 64 ? 4 : (pairs > 32 ? 2 : 1);
 }
 
 int launch_half_sweep(ps_ctx *c, const double *rhs, double *p, double omega, int colour)
@@ -259,10 +271,12 @@ int run_sweeps_untimed(ps_ctx *c, const double *rhs, double *p, double **cur, do
     if (otf && !c->have_rho) return PS_ESTATE;
     const double c2x = 2.0 * (1.0 / (c->dx * c->dx)), c2y = 2.0 * (1.0 / (c->dy * c->dy)),
                  c2z = 2.0 * (1.0 / (c->dz * c->dz));
+    const bool pdl_on = launch_dependent(c);
+    c->fused.pace_window = launch_pace_window(c);
     for (int left = n; left > 0; --left) {
         // every sweep after the first of the batch is a dependent launch: its predecessor in the
         // stream is a sweep, which writes none of the coefficient, rho or rhs boxes
-        const bool dep = c->pdl && left < n;
+        const bool dep = pdl_on && left < n;
         cudaError_t e =
             otf ? ps::zm_launch_otf(c->fused, c->g, c->rho, c2x, c2y, c2z, rhs, src, dst, omega,
                                     c->stream, dep)
@@ -342,7 +356,8 @@ int ps_create(ps_ctx **out, int nx, int ny, int nz, double dx, double dy, double
     if (!c->ev) { delete c; return PS_ENOMEM; }
     c->dx = dx; c->dy = dy; c->dz = dz;
     c->K = 50;
-    c->pdl = true;
+    c->pdl_mode = -1;
+    c->pace_mode = -1;
     c->sm_count = sms;
     c->coop = coop;
     c->nparts = nparts_for(c->g.cells());
@@ -456,16 +471,16 @@ int ps_set_launch_options(ps_ctx *c, int dependent_launch, int pace_window)
     if (!c || !c->fused.ok) return PS_EINVAL;
     if (dependent_launch < -1 || dependent_launch > 1 || pace_window < -1 || pace_window > 64)
         return PS_EINVAL;
-    if (dependent_launch >= 0) c->pdl = dependent_launch != 0;
-    if (pace_window >= 0) c->fused.pace_window = pace_window;
+    c->pdl_mode = dependent_launch;
+    c->pace_mode = pace_window;
     return PS_OK;
 }
 
 int ps_get_launch_options(const ps_ctx *c, int *dependent_launch, int *pace_window)
 {
     if (!c || !c->fused.ok) return PS_EINVAL;
-    if (dependent_launch) *dependent_launch = c->pdl ? 1 : 0;
-    if (pace_window) *pace_window = c->fused.pace_window;
+    if (dependent_launch) *dependent_launch = launch_dependent(c) ? 1 : 0;
+    if (pace_window) *pace_window = launch_pace_window(c);
     return PS_OK;
 }
 
@@ -1044,18 +1059,10 @@ int ps_rhs_from_velocity(ps_ctx *c, const double *ux_dev, const double *uy_dev,
     if (!aligned16(ux_dev, uy_dev, uz_dev, rhs_dev)) return PS_EINVAL;
     const ps::Spacing h{c->dx, c->dy, c->dz};
     int kz = 0;
-    const int wx = zs_wx(c);
-    if (c->g.nx % 2 == 0 && c->g.ny <= 65535) {
-        const dim3 grid = zs_grid(c, wx, &kz);
-        if (wx == 4)
-            ps::ps_rhs_from_velocity_pair_kernel<4><<<grid, ps::ZS_THREADS, 0, c->stream>>>(
-                c->g, h, ux_dev, uy_dev, uz_dev, dt, rhs_dev, kz);
-        else if (wx == 2)
-            ps::ps_rhs_from_velocity_pair_kernel<2><<<grid, ps::ZS_THREADS, 0, c->stream>>>(
-                c->g, h, ux_dev, uy_dev, uz_dev, dt, rhs_dev, kz);
-        else
-            ps::ps_rhs_from_velocity_pair_kernel<1><<<grid, ps::ZS_THREADS, 0, c->stream>>>(
-                c->g, h, ux_dev, uy_dev, uz_dev, dt, rhs_dev, kz);
+    if (c->g.nx % 2 == 0 && c->g.ny <= 65535 * ps::ZS_TY) {
+        const dim3 grid = zs_grid(c, 32, &kz);
+        ps::ps_rhs_from_velocity_pair_kernel<<<grid, ps::ZS_TX * ps::ZS_TY, 0, c->stream>>>(
+            c->g, h, ux_dev, uy_dev, uz_dev, dt, rhs_dev, kz);
     } else
         ps::ps_rhs_from_velocity_kernel<<<grid_for(c, c->g.cells(), 256), 256, 0, c->stream>>>(
             c->g, h, ux_dev, uy_dev, uz_dev, dt, rhs_dev);
@@ -1088,18 +1095,10 @@ int ps_face_divergence(ps_ctx *c, const double *ux_dev, const double *uy_dev, co
     if (!c->have_coef) return PS_ESTATE;
     const ps::Spacing h{c->dx, c->dy, c->dz};
     int kz = 0;
-    const int wx = zs_wx(c);
-    if (c->g.nx % 2 == 0 && c->g.ny <= 65535) {
-        const dim3 grid = zs_grid(c, wx, &kz);
-        if (wx == 4)
-            ps::ps_face_divergence_pair_kernel<4><<<grid, ps::ZS_THREADS, 0, c->stream>>>(
-                c->g, h, c->ax, c->ay, c->az, ux_dev, uy_dev, uz_dev, p_dev, dt, div_dev, kz);
-        else if (wx == 2)
-            ps::ps_face_divergence_pair_kernel<2><<<grid, ps::ZS_THREADS, 0, c->stream>>>(
-                c->g, h, c->ax, c->ay, c->az, ux_dev, uy_dev, uz_dev, p_dev, dt, div_dev, kz);
-        else
-            ps::ps_face_divergence_pair_kernel<1><<<grid, ps::ZS_THREADS, 0, c->stream>>>(
-                c->g, h, c->ax, c->ay, c->az, ux_dev, uy_dev, uz_dev, p_dev, dt, div_dev, kz);
+    if (c->g.nx % 2 == 0 && c->g.ny <= 65535 * ps::ZS_TY) {
+        const dim3 grid = zs_grid(c, 8, &kz);
+        ps::ps_face_divergence_pair_kernel<<<grid, ps::ZS_TX * ps::ZS_TY, 0, c->stream>>>(
+            c->g, h, c->ax, c->ay, c->az, ux_dev, uy_dev, uz_dev, p_dev, dt, div_dev, kz);
     } else
         ps::ps_face_divergence_kernel<<<grid_for(c, c->g.cells(), 256), 256, 0, c->stream>>>(
             c->g, h, c->ax, c->ay, c->az, ux_dev, uy_dev, uz_dev, p_dev, dt, div_dev);

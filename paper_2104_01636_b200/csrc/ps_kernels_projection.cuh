@@ -144,7 +144,7 @@ __device__ __forceinline__ PairCell pair_cell(const Grid &g, unsigned h)
 // plane of those fields is loaded once per chunk instead of three times.  Read through L1/L2 like
 // the one-cell kernels, the z neighbours alone were 1/3 of the load instructions and of the L2
 // traffic, and the kernels ran at 0.8 of the HBM roofline, bound by L2 bandwidth.
-constexpr int ZS_THREADS = 256;   // 8 warps: WX warps along x (32 x-pairs each) x 8 / WX rows
+constexpr int ZS_TX = 32, ZS_TY = 8;
 
 struct ZsCell { int i, j; size_t n; };     // left cell of the pair and its linear index on plane k
 
@@ -211,13 +211,11 @@ __device__ __forceinline__ void face_gradients_pair(const Grid &g, const Spacing
 }
 
 // Grid of the z-marching kernels: x tiles, y tiles, z chunks of kz planes.
-template <int WX>
 __device__ __forceinline__ bool zs_setup(const Grid &g, int kz, ZsCell &c, int &k0, int &k1,
                                          size_t &plane, size_t &nzm)
 {
-    const int warp = (int)(threadIdx.x >> 5);
-    c.i = 2 * (((int)blockIdx.x * WX + warp % WX) * 32 + (int)(threadIdx.x & 31u));
-    c.j = (int)blockIdx.y * (8 / WX) + warp / WX;
+    c.i = 2 * ((int)blockIdx.x * ZS_TX + (int)(threadIdx.x & 31u));
+    c.j = (int)blockIdx.y * ZS_TY + (int)(threadIdx.x >> 5);
     k0 = (int)blockIdx.z * kz;
     k1 = k0 + kz < g.nz ? k0 + kz : g.nz;
     if (c.i >= g.nx || c.j >= g.ny || k0 >= k1) return false;
@@ -227,8 +225,7 @@ __device__ __forceinline__ bool zs_setup(const Grid &g, int kz, ZsCell &c, int &
     return true;
 }
 
-template <int WX>
-__global__ void __launch_bounds__(ZS_THREADS)
+__global__ void __launch_bounds__(ZS_TX * ZS_TY)
 ps_rhs_from_velocity_pair_kernel(Grid g, Spacing h, const double *__restrict__ ux,
                                  const double *__restrict__ uy, const double *__restrict__ uz,
                                  double dt, double *__restrict__ rhs, int kz)
@@ -236,7 +233,7 @@ ps_rhs_from_velocity_pair_kernel(Grid g, Spacing h, const double *__restrict__ u
     ZsCell c;
     int k0, k1;
     size_t plane, nzm;
-    if (!zs_setup<WX>(g, kz, c, k0, k1, plane, nzm)) return;
+    if (!zs_setup(g, kz, c, k0, k1, plane, nzm)) return;
     double2 UZm = ld2(uz + nzm), UZ = ld2(uz + c.n);
     for (int k = k0; k < k1; ++k, c.n += plane) {
         const size_t nzp = (k + 1 < g.nz) ? c.n + plane : c.n - plane * (size_t)(g.nz - 1);
@@ -251,8 +248,7 @@ ps_rhs_from_velocity_pair_kernel(Grid g, Spacing h, const double *__restrict__ u
     }
 }
 
-template <int WX>
-__global__ void __launch_bounds__(ZS_THREADS, 3)
+__global__ void __launch_bounds__(ZS_TX * ZS_TY, 3)
 ps_face_divergence_pair_kernel(Grid g, Spacing h, const double *__restrict__ ax,
                                const double *__restrict__ ay, const double *__restrict__ az,
                                const double *__restrict__ ux, const double *__restrict__ uy,
@@ -262,7 +258,7 @@ ps_face_divergence_pair_kernel(Grid g, Spacing h, const double *__restrict__ ax,
     ZsCell c;
     int k0, k1;
     size_t plane, nzm;
-    if (!zs_setup<WX>(g, kz, c, k0, k1, plane, nzm)) return;
+    if (!zs_setup(g, kz, c, k0, k1, plane, nzm)) return;
     double2 UZm = ld2(uz + nzm), UZ = ld2(uz + c.n);
     double2 Pzm = ld2(p + nzm), P = ld2(p + c.n);
     double2 AZm = ld2(az + nzm);

@@ -19,7 +19,7 @@ BYTES_PER_UPDATE = {"twopass": 80.0, "fused": 48.0, "fused_otf": 32.0, "resident
 
 
 def run_config(cfg: int, max_sweeps: int, to_tol: bool, kernel: int, mg_cycles: int = 1000,
-               fixed_override: int = 0):
+               fixed_override: int = 0, launch_options=(-1, -1), mg: bool = True):
     import torch
     from . import binding, workload as wl
     w = wl.make_config(cfg)
@@ -32,6 +32,9 @@ def run_config(cfg: int, max_sweeps: int, to_tol: bool, kernel: int, mg_cycles: 
         s.set_kernel(kernel)
         kname = binding.KERNEL_NAMES[s.get_kernel()]
         out["kernel"] = kname
+        if kname in ("fused", "fused_otf"):
+            s.set_launch_options(*launch_options)
+            out["dependent_launch"], out["pace_window"] = s.get_launch_options()
         s.set_fraction(F_d, w.rho_l, w.rho_g)
         s.sweeps(rhs_d, p_d, w.omega, min(fixed, 20))          # warm-up
         torch.cuda.synchronize()
@@ -55,6 +58,8 @@ def run_config(cfg: int, max_sweeps: int, to_tol: bool, kernel: int, mg_cycles: 
             torch.cuda.synchronize()
             out.update(tol_seconds=time.perf_counter() - t0, tol_sweeps=info.sweeps,
                        tol_converged=bool(info.converged), tol_res_rel=info.res_rel)
+        if not mg:
+            return out
         # multigrid accelerated solve, binding defaults, every config; an untimed
         # two-cycle warm-up first (level memory, lazy loading of the multigrid kernels), as in
         # bench.py: a time stepper pays those once, not per solve
@@ -155,8 +160,9 @@ def to_markdown(rows) -> str:
         body += (f"| {r['config']} | {r['workload']} | {r['kernel']} | {r['fixed_sweeps']} | "
                  f"{r['fixed_ms']:.2f} | {r['gcell_per_s']:.1f} | {r['model_gb_per_s']:.0f} | "
                  f"{r['res_rel_after_fixed']:.3e} | {tol} | "
-                 f"{r['mg_cycles']}{'' if r['mg_converged'] else ' (not converged)'} "
-                 f"({r['mg_levels']}) | {r['mg_seconds']:.3f} | {r['mg_res_rel']:.3e} |\n")
+                 + (f"{r['mg_cycles']}{'' if r['mg_converged'] else ' (not converged)'} "
+                    f"({r['mg_levels']}) | {r['mg_seconds']:.3f} | {r['mg_res_rel']:.3e} |\n"
+                    if "mg_cycles" in r else "- | - | - |\n"))
     return head + body
 
 
@@ -170,6 +176,11 @@ def main(argv=None):
     ap.add_argument("--mg-cycles", type=int, default=1000, help="cap of multigrid cycles")
     ap.add_argument("--sweeps", type=int, default=0, help="fixed-sweep count (default: the config's)")
     ap.add_argument("--kernel", default="auto", choices=["auto", "twopass", "fused", "fused_otf"])
+    ap.add_argument("--no-mg", action="store_true", help="skip the multigrid legs")
+    ap.add_argument("--pace-window", type=int, default=-1,
+                    help="fused kernel: pacing window (0 = off, -1 = library choice)")
+    ap.add_argument("--dependent-launch", type=int, default=-1,
+                    help="fused kernel: dependent launches 0/1 (-1 = library choice)")
     ap.add_argument("--md", default="", help="also write the table to this file")
     ap.add_argument("--kernel-rates", action="store_true",
                     help="only time the single-pass kernels on config 4 and print their rates")
@@ -203,7 +214,9 @@ def main(argv=None):
     rows = []
     for cfg in [int(c) for c in args.configs.split(",")]:
         r = run_config(cfg, args.max_sweeps, to_tol=(not args.no_tol and str(cfg) in args.sor_tol_configs.split(',')), kernel=kernel,
-                       mg_cycles=args.mg_cycles, fixed_override=args.sweeps)
+                       mg_cycles=args.mg_cycles, fixed_override=args.sweeps,
+                       launch_options=(args.dependent_launch, args.pace_window),
+                       mg=not args.no_mg)
         print(json.dumps(r), file=sys.stderr, flush=True)
         rows.append(r)
     md = to_markdown(rows)

@@ -104,7 +104,7 @@ def test_checked_kernel_long_run_and_multigrid(torch_cuda, B, checked, ora):
         s.sweeps(rhs_d, p_d, w.omega, 300)
         assert s.debug_read()[0] == 0, s.debug_read()
         assert int(np.count_nonzero(p_d.cpu().numpy() != p_ora)) == 0
-        prm = dict(levels=6, nu1=0, nu2=2, coarse_sweeps=30, gamma=1, omega_s=1.75, nu_growth=4, nu_max=16)
+        prm = dict(B.MG_DEFAULTS)
         q_ora = np.zeros_like(w.rhs)
         ora.mg_solve(coef, w.rhs, q_ora, 3, 0.0, **prm)
         s.mg_setup(**prm)

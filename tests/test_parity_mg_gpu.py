@@ -90,7 +90,9 @@ PARAMS = [
     dict(levels=3, nu1=2, nu2=2, coarse_sweeps=30, gamma=2, omega_s=1.3, nu_growth=1, nu_max=64),
     dict(levels=1, nu1=0, nu2=0, coarse_sweeps=5, gamma=1, omega_s=1.5, nu_growth=1, nu_max=64),     # plain SOR
     dict(levels=99, nu1=2, nu2=1, coarse_sweeps=40, gamma=1, omega_s=1.6, nu_growth=4, nu_max=16),
-    dict(levels=99, nu1=0, nu2=2, coarse_sweeps=30, gamma=1, omega_s=1.75, nu_growth=4, nu_max=16),  # the binding defaults
+    dict(levels=99, nu1=0, nu2=2, coarse_sweeps=30, gamma=1, omega_s=1.75, nu_growth=4, nu_max=16),  # round 1's defaults
+    dict(levels=99, nu1=1, nu2=2, coarse_sweeps=9, gamma=1, omega_s=1.45, omega_c=1.9, nu_growth=3, nu_max=12),  # two relaxation factors
+    None,                                                                                             # binding.MG_DEFAULTS
 ]
 
 
@@ -98,6 +100,7 @@ PARAMS = [
 @pytest.mark.parametrize("prm", PARAMS)
 def test_cycles_bitwise(torch_cuda, B, ora, shape, prm):
     w = workload(*shape)
+    prm = dict(B.MG_DEFAULTS) if prm is None else prm
     coef = ora.coefficients(w.F, w.rho_l, w.rho_g, w.dx, w.dy, w.dz)
     p_o = np.zeros_like(w.rhs)
     io = ora.mg_solve(coef, w.rhs, p_o, 3, 0.0, **prm)
@@ -138,7 +141,8 @@ def test_fused_norm_path_defaults_to_tolerance(torch_cuda, B, ora):
     bitwise, norms to 1e-10 (a different fixed summation tree), at least one cycle even from a
     converged start, max_cycles honoured, max_cycles = 0 only measures."""
     w = wl.make_config(1)
-    prm = dict(levels=6, nu1=0, nu2=2, coarse_sweeps=30, gamma=1, omega_s=1.75, nu_growth=4, nu_max=16)
+    prm = dict(B.MG_DEFAULTS)
+    assert prm["nu1"] == 0                                       # the fused-norm path
     coef = ora.coefficients(w.F, w.rho_l, w.rho_g, w.dx, w.dy, w.dz)
     p_o = np.zeros_like(w.rhs)
     io = ora.mg_solve(coef, w.rhs, p_o, 200, 1e-8, **prm)
@@ -198,12 +202,14 @@ def test_config3_three_cycles_and_state_errors(torch_cuda, B, ora):
 
 
 def test_diverging_parameters_stop_early(torch_cuda, B):
-    """V(0,2) with omega_s = 1.9 diverges; ps_mg_solve must not grind through
-    max_cycles on infinities: it stops at the first cycle whose norm is not finite."""
+    """V(0,2) with 2 / 8 / 16 sweeps per level and one relaxation factor of 1.9 diverges
+    (DESIGN.md §12); ps_mg_solve must not grind through max_cycles on infinities: it stops at the
+    first cycle whose norm is not finite."""
     w = wl.make_config(1)
     with B.PoissonSolver(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz) as s:
         s.set_fraction(dev(torch_cuda, w.F), w.rho_l, w.rho_g)
-        s.mg_setup(omega_s=1.9)
+        s.mg_setup(levels=6, nu1=0, nu2=2, coarse_sweeps=30, gamma=1, omega_s=1.9, omega_c=1.9,
+                   nu_growth=4, nu_max=16)
         p_d = torch_cuda.zeros(w.rhs.shape, dtype=torch_cuda.float64, device="cuda")
         info = s.mg_solve(dev(torch_cuda, w.rhs), p_d, 100000, 1e-8)
         assert not info.converged and info.sweeps < 100000

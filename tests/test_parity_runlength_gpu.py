@@ -22,8 +22,6 @@ from paper_2104_01636_b200 import workload as wl
 pytestmark = pytest.mark.gpu
 
 P_TOL, NORM_TOL, TOL = 1e-12, 1e-10, 1e-8
-MG_DEFAULTS = dict(levels=6, nu1=0, nu2=2, coarse_sweeps=30, gamma=1, omega_s=1.75, nu_growth=4,
-                   nu_max=16)
 
 
 @pytest.fixture(scope="module")
@@ -101,10 +99,10 @@ def test_default_multigrid_bitwise_and_to_tolerance(torch_cuda, B, ora, cfg, cyc
     w = config(cfg)
     coef = ora.coefficients(w.F, w.rho_l, w.rho_g, w.dx, w.dy, w.dz)
     p_o = np.zeros_like(w.rhs)
-    io = ora.mg_solve(coef, w.rhs, p_o, cycles, 0.0, **MG_DEFAULTS)
+    io = ora.mg_solve(coef, w.rhs, p_o, cycles, 0.0, **B.MG_DEFAULTS)
     with B.PoissonSolver(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz) as s:
         s.set_fraction(dev(torch_cuda, w.F), w.rho_l, w.rho_g)
-        assert s.mg_setup() == 6                                  # the defaults
+        assert s.mg_setup() == B.MG_DEFAULTS["levels"] == 6       # the defaults
         rhs_d = dev(torch_cuda, w.rhs)
         p_d = torch_cuda.zeros_like(rhs_d)
         ig = s.mg_solve(rhs_d, p_d, cycles, 0.0)
