@@ -20,14 +20,15 @@ KERNEL_AUTO, KERNEL_TWOPASS, KERNEL_FUSED, KERNEL_RESIDENT, KERNEL_FUSED_OTF = 0
 KERNEL_NAMES = {KERNEL_AUTO: "auto", KERNEL_TWOPASS: "twopass", KERNEL_FUSED: "fused",
                 KERNEL_RESIDENT: "resident", KERNEL_FUSED_OTF: "fused_otf"}
 
-# Multigrid parameters `mg_setup()` uses when none are given (measured fastest to
-# 1e-8 on the bubbly configs among ~500 settings, profiles/r02_mg_tuning.md): V(0,2) -- no
-# pre-smoothing, 2 post-smoothing sweeps on the finest level at omega_s = 1.5 --, 32 sweeps at
-# omega_c = 1.95 on every coarser level, 10 on the coarsest of 6.  omega_c = 1.97 still converges on
-# every config, 1.98 does not.  The one place they are written down: bench.py, report.py and the
-# parity tests take them from here.
-MG_DEFAULTS = dict(levels=6, nu1=0, nu2=2, coarse_sweeps=10, gamma=1, omega_s=1.5, omega_c=1.95,
-                   nu_growth=16, nu_max=32)
+# Multigrid parameters `mg_setup()` uses when none are given (chosen among ~700
+# settings scanned on the five configs, profiles/r02_mg_tuning.md): V(0,2) -- no pre-smoothing, 2
+# post-smoothing sweeps on the finest level at omega_s = 1.4 --, 48 sweeps at omega_c = 1.97 on
+# every coarser level, 10 on the coarsest of 6: 16-21 cycles to 1e-8 on all five configs.
+# omega_c = 1.98 is ~10 % faster and 1.985 still converges on every config and seed tried; 1.99 does
+# not on all.  The one place they are written down: bench.py, report.py and the parity tests take
+# them from here.
+MG_DEFAULTS = dict(levels=6, nu1=0, nu2=2, coarse_sweeps=10, gamma=1, omega_s=1.4, omega_c=1.97,
+                   nu_growth=24, nu_max=48)
 
 # every symbol include/ps_poisson.h declares (tests check the library exports each one)
 SYMBOLS = ("ps_create", "ps_destroy", "ps_workspace_bytes", "ps_set_workspace", "ps_set_stream",

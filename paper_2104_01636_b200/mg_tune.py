@@ -2,7 +2,7 @@
 
     python -m paper_2104_01636_b200.mg_tune --configs 3,4 --omega-s 1.4,1.5,1.6 \
         --omega-c 1.9,1.95 --nu-growth 4,16 --nu-max 16,32 [--nu 0:2,1:1] [--coarse-sweeps 10,30] \
-        [--levels 6] [--gamma 1] [--max-cycles 400] [--md FILE]
+        [--levels 6] [--gamma 1] [--max-cycles 400] [--seed-offset 0] [--md FILE]
 
 Every combination of the listed values is run through `ps_mg_setup` + `ps_mg_solve(tol = 1e-8)`
 from p = 0 (after one untimed warm-up solve per config, so that level memory and kernels are
@@ -40,6 +40,8 @@ def main(argv=None):
     ap.add_argument("--nu-growth", default="16")
     ap.add_argument("--nu-max", default="32")
     ap.add_argument("--max-cycles", type=int, default=400)
+    ap.add_argument("--seed-offset", type=int, default=0,
+                    help="another bubble arrangement and rhs of the same recipe (workload.make_config)")
     ap.add_argument("--md", default="")
     args = ap.parse_args(argv)
     import torch
@@ -55,7 +57,7 @@ def main(argv=None):
                                   _ints(args.nu_growth), _ints(args.nu_max)))
     results = {}
     for cfg in cfgs:
-        w = wl.make_config(cfg)
+        w = wl.make_config(cfg, seed_offset=args.seed_offset)
         F_d = torch.from_numpy(w.F).cuda()
         rhs_d = torch.from_numpy(w.rhs).cuda()
         p_d = torch.zeros_like(rhs_d)
