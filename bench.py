@@ -44,7 +44,10 @@ UNIT = "Gcell-updates/s"
 #   fused_otf: the same with rho (8 B) in place of ax, ay, az (24 B) = 32 B per cell-update
 #   resident: many sweeps per cooperative launch on an L2-resident grid; 80 B per cell-update of
 #             L2 (not HBM) traffic -- reported, but not an HBM roofline
-ALGO_BYTES_PER_UPDATE = {"twopass": 80.0, "fused": 48.0, "fused_otf": 32.0, "resident": 80.0}
+#   cluster:  many sweeps per launch with the grid in the shared memory of one cluster; the same
+#             80 B per cell-update, of SHARED-MEMORY traffic -- reported, not an HBM roofline
+ALGO_BYTES_PER_UPDATE = {"twopass": 80.0, "fused": 48.0, "fused_otf": 32.0, "resident": 80.0,
+                         "cluster": 80.0}
 
 
 # Plain red-black SOR (row a5 alone) on the configs where a live run to 1e-8 does not fit a bench:
@@ -64,7 +67,7 @@ def parse_args():
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json config 1..5 (default 4)")
     ap.add_argument("--sweeps", type=int, default=0, help="sweeps per step (default: the config's)")
     ap.add_argument("--kernel", default="auto",
-                    choices=["auto", "twopass", "fused", "resident", "fused_otf"])
+                    choices=["auto", "twopass", "fused", "resident", "fused_otf", "cluster"])
     ap.add_argument("--no-mg", action="store_true", help="skip the time-to-1e-8 legs")
     ap.add_argument("--sor-sweeps", type=int, default=-1,
                     help="cap of the live plain-SOR solve to 1e-8 (default: 1e6 for grids up to "
@@ -256,7 +259,7 @@ def run_ours(args, rank):
     shape = (w.nz, w.ny, w.nx)
     kernel = {"auto": binding.KERNEL_AUTO, "twopass": binding.KERNEL_TWOPASS,
               "fused": binding.KERNEL_FUSED, "fused_otf": binding.KERNEL_FUSED_OTF,
-              "resident": binding.KERNEL_RESIDENT}[args.kernel]
+              "resident": binding.KERNEL_RESIDENT, "cluster": binding.KERNEL_CLUSTER}[args.kernel]
 
     F_h = torch.from_numpy(w.F).pin_memory()
     rhs_h = torch.from_numpy(w.rhs).pin_memory()
@@ -398,7 +401,7 @@ def run_ours(args, rank):
                                    if sweep_ms > 0 else None,
         "gpu_launches": launches,
         "clocks": clk,
-        "roofline": {"bound": "hbm" if kname != "resident" else "l2 (grid is L2-resident: not an "
+        "roofline": {"bound": "hbm" if kname not in ("resident", "cluster") else "l2 (grid is L2-resident: not an "
                                                                   "HBM measurement)",
                      "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_src,

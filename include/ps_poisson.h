@@ -60,6 +60,11 @@ extern "C" {
                                /* per pair of updates).  Select it    */
                                /* BEFORE ps_set_fraction (which then also stores rho), else */
                                /* the sweeps return PS_ESTATE.                              */
+#define PS_KERNEL_CLUSTER  5   /* grids that fit the shared memory of one thread-block      */
+                               /* cluster (<= 16 CTAs x 227 KB: about 65 k cells): n sweeps */
+                               /* in ONE launch, p and the coefficients on chip, z-slab     */
+                               /* neighbours through distributed shared memory, one cluster */
+                               /* barrier per half-sweep, in place, any nx,ny>=1            */
 
 typedef struct ps_ctx ps_ctx;   /* opaque; one per grid */
 

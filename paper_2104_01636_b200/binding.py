@@ -17,8 +17,10 @@ from . import build as _build
 
 PS_OK, PS_EINVAL, PS_ESTATE, PS_ECUDA, PS_ENOMEM = 0, -1, -2, -3, -4
 KERNEL_AUTO, KERNEL_TWOPASS, KERNEL_FUSED, KERNEL_RESIDENT, KERNEL_FUSED_OTF = 0, 1, 2, 3, 4
+KERNEL_CLUSTER = 5
 KERNEL_NAMES = {KERNEL_AUTO: "auto", KERNEL_TWOPASS: "twopass", KERNEL_FUSED: "fused",
-                KERNEL_RESIDENT: "resident", KERNEL_FUSED_OTF: "fused_otf"}
+                KERNEL_RESIDENT: "resident", KERNEL_FUSED_OTF: "fused_otf",
+                KERNEL_CLUSTER: "cluster"}
 
 # Multigrid parameters `mg_setup()` uses when none are given (chosen among ~700
 # settings scanned on the five configs, profiles/r02_mg_tuning.md): V(0,2) -- no pre-smoothing, 2

@@ -15,6 +15,7 @@
 #include "ps_kernels_zmarch.cuh"
 #include "ps_kernels_mg.cuh"
 #include "ps_kernels_resident.cuh"
+#include "ps_kernels_cluster.cuh"
 #include "ps_kernels_projection.cuh"
 
 namespace {
@@ -57,6 +58,7 @@ struct ps_ctx {
     bool have_rho;         // rho field of the on-the-fly sweep variant is current
     int sm_count;
     int coop;              // device supports cooperative launches
+    int cluster_c;         // CTAs of the cluster kernel for this grid (0: does not fit / no device support)
     int pdl_mode;          // dependent launches of the fused sweeps: -1 automatic, 0 off, 1 on
     int pace_mode;         // pacing window of the fused sweeps: -1 automatic, 0 off, n
     long long launches;
@@ -164,13 +166,15 @@ int resolve_variant(const ps_ctx *c, int req)
     const bool fused_ok = c->fused.ok;
     // small grids live in L2 and are bound by launch / pipeline start-up latency: many sweeps per
     // cooperative launch win there (measured cross-over between 65 k and 524 k cells)
+    if (req == PS_KERNEL_AUTO && c->cluster_c > 0) return PS_KERNEL_CLUSTER;
     if (req == PS_KERNEL_AUTO && c->coop && c->g.cells() <= (size_t)ps_resident_max_cells)
         return PS_KERNEL_RESIDENT;
     if (req == PS_KERNEL_AUTO) return fused_ok ? PS_KERNEL_FUSED : PS_KERNEL_TWOPASS;
     if (req == PS_KERNEL_FUSED && !fused_ok) return -1;
     if (req == PS_KERNEL_FUSED_OTF && !fused_ok) return -1;
     if (req == PS_KERNEL_RESIDENT && !c->coop) return -1;
-    if (req < PS_KERNEL_AUTO || req > PS_KERNEL_FUSED_OTF) return -1;
+    if (req == PS_KERNEL_CLUSTER && c->cluster_c == 0) return -1;
+    if (req < PS_KERNEL_AUTO || req > PS_KERNEL_CLUSTER) return -1;
     return req;
 }
 
@@ -246,6 +250,12 @@ int run_sweeps_untimed(ps_ctx *c, const double *rhs, double *p, double **cur, do
             if (rc) return rc;
         }
         return PS_OK;
+    }
+    if (c->variant == PS_KERNEL_CLUSTER) {
+        const cudaError_t e = ps::cl_launch(c->g, c->cluster_c, c->ax, c->ay, c->az, rhs, *cur,
+                                            omega, n, c->stream);
+        c->launches++;
+        return e == cudaSuccess ? PS_OK : cuda_fail(e);
     }
     if (c->variant == PS_KERNEL_RESIDENT) {
         const size_t items = (size_t)((c->g.nx + 1) / 2) * c->g.ny * c->g.nz;
@@ -371,6 +381,7 @@ int ps_create(ps_ctx **out, int nx, int ny, int nz, double dx, double dy, double
         delete c;
         return cuda_fail(e);
     }
+    c->cluster_c = ps::cl_plan(c->g);
     c->variant_req = PS_KERNEL_AUTO;
     c->variant = resolve_variant(c, PS_KERNEL_AUTO);
     *out = c;

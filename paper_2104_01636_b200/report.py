@@ -15,7 +15,8 @@ import json
 import sys
 import time
 
-BYTES_PER_UPDATE = {"twopass": 80.0, "fused": 48.0, "fused_otf": 32.0, "resident": 80.0}
+BYTES_PER_UPDATE = {"twopass": 80.0, "fused": 48.0, "fused_otf": 32.0, "resident": 80.0,
+                    "cluster": 80.0}
 
 
 def run_config(cfg: int, max_sweeps: int, to_tol: bool, kernel: int, mg_cycles: int = 1000,

@@ -50,12 +50,13 @@ def variants_for(B, w, tunings=((1, 0, -1, -1), (1, 1, 0, 0), (1, 2, 1, 0), (1, 
     chunk items) and with its launch options on and off (-1: the library defaults)."""
     out = []
     with B.PoissonSolver(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, workspace=False) as s:
-        for v in (B.KERNEL_TWOPASS, B.KERNEL_RESIDENT, B.KERNEL_FUSED_OTF, B.KERNEL_FUSED):
+        for v in (B.KERNEL_TWOPASS, B.KERNEL_RESIDENT, B.KERNEL_CLUSTER, B.KERNEL_FUSED_OTF,
+                  B.KERNEL_FUSED):
             try:
                 s.set_kernel(v)
             except B.PsError:
                 continue
-            if v in (B.KERNEL_TWOPASS, B.KERNEL_RESIDENT):
+            if v in (B.KERNEL_TWOPASS, B.KERNEL_RESIDENT, B.KERNEL_CLUSTER):
                 out.append((v, 0, 0, -1, -1))
                 continue
             for rpt, chunks, dep, window in tunings:
@@ -73,7 +74,7 @@ def make_solver(B, w, variant=None):
     if variant is not None:
         kernel, rpt, chunks, dep, window = variant
         s.set_kernel(kernel)
-        if kernel not in (B.KERNEL_TWOPASS, B.KERNEL_RESIDENT):
+        if kernel not in (B.KERNEL_TWOPASS, B.KERNEL_RESIDENT, B.KERNEL_CLUSTER):
             s.set_tuning(rpt, chunks)
             s.set_launch_options(dep, window)
     return s
@@ -519,9 +520,9 @@ def test_unaligned_pointers_are_rejected_everywhere(torch_cuda, B, ora):
     ora.sweep(coef, w.rhs, p_ora, w.omega, 3)
     lib = B.load()
     ptr = lambda t: ctypes.c_void_p(t.data_ptr())
-    for kernel in (B.KERNEL_TWOPASS, B.KERNEL_FUSED, B.KERNEL_RESIDENT):
+    for kernel in (B.KERNEL_TWOPASS, B.KERNEL_FUSED, B.KERNEL_RESIDENT, B.KERNEL_CLUSTER):
         with B.PoissonSolver(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz) as s:
-            s.set_kernel(kernel)
+            s.set_kernel(kernel)                         # 40 x 36 x 24 fits one cluster
             F_d, rhs_d = to_dev(torch_cuda, w.F), to_dev(torch_cuda, w.rhs)
             p_d = torch_cuda.zeros_like(rhs_d)
             bad_F, bad_rhs, bad_p = odd(w.F), odd(w.rhs), odd()
