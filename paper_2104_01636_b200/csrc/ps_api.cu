@@ -146,7 +146,7 @@ int ensure_workspace(ps_ctx *c)
 //  * dependent launches pay where a launch is short (config 2, 8 steps per CTA: 10.2 -> 6.9 us per
 //    sweep; config 3, 35 steps: 37.0 -> 35.3) and cost 4 % in sustained runs of long launches
 //    (config 4, 270 steps: 129.1 -> 124.0 Gcell-updates/s at the power cap);
-//  * pacing cuts the DRAM traffic of cold bursts at full clocks (config 5: 1.19 -> 1.06 x
+//  * pacing cuts the DRAM traffic of cold bursts at full clocks (config 5: 1.19 -> 1.03 x
 //    algorithmic, 112 -> 137 Gcell-updates/s) but costs 8 % in sustained runs on every config
 //    (config 5: 131.3 -> 120.4), the regime a solver lives in: off unless asked for.
 constexpr int ps_pdl_max_steps = 96;      // dependent launches up to this many steps per CTA

@@ -104,6 +104,16 @@ def test_checked_kernel_long_run_and_multigrid(torch_cuda, B, checked, ora):
         s.sweeps(rhs_d, p_d, w.omega, 300)
         assert s.debug_read()[0] == 0, s.debug_read()
         assert int(np.count_nonzero(p_d.cpu().numpy() != p_ora)) == 0
+        # the launch options the library would not pick by itself: dependent launches and pacing
+        # both on, both off (the producer then waits on the pacing counter / the grid dependency
+        # before it issues the p planes; the ring tags still have to come out right)
+        for dep, window in ((1, 2), (1, 1), (0, 0)):
+            s.set_launch_options(dep, window)
+            p_d.zero_()
+            s.sweeps(rhs_d, p_d, w.omega, 300)
+            assert s.debug_read()[0] == 0, (dep, window, s.debug_read())
+            assert int(np.count_nonzero(p_d.cpu().numpy() != p_ora)) == 0, (dep, window)
+        s.set_launch_options(-1, -1)
         prm = dict(B.MG_DEFAULTS)
         q_ora = np.zeros_like(w.rhs)
         ora.mg_solve(coef, w.rhs, q_ora, 3, 0.0, **prm)
