@@ -131,10 +131,11 @@ int ps_get_tuning(const ps_ctx *c, int *rows_per_thread, int *z_chunks, int *til
  *   pace_window       n > 0: no CTA issues a stage more than n stages ahead of the mean over all
  *                     CTAs of the launch, which keeps the halo rows and columns that neighbouring
  *                     tiles share inside L2 (one global counter, one atomic and one load per CTA
- *                     and plane); 0: CTAs run free.
+ *                     and four planes); 0: CTAs run free.
  * -1 (the default of both) leaves the choice to the library: dependent launches where a launch
- * is short (up to 96 z steps per CTA), no pacing (it wins cold bursts at full clocks, up to 25 %
- * on the 151 M-cell duct, and loses 8 % in sustained runs at the power cap).  ps_get_launch_options
+ * is short (up to 96 z steps per CTA), pacing with a window of 2 where it is longer (it wins
+ * cold bursts at full clocks, 5 % on the 34 M-cell and 24 % on the 151 M-cell duct, and is neutral
+ * in sustained runs at the power cap).  ps_get_launch_options
  * returns the settings in effect.  PS_EINVAL: no fused kernel for this grid, values out of
  * range (pace_window > 64). */
 int ps_set_launch_options(ps_ctx *c, int dependent_launch, int pace_window);

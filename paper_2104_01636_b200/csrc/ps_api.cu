@@ -147,9 +147,13 @@ int ensure_workspace(ps_ctx *c)
 //    sweep; config 3, 35 steps: 37.0 -> 35.3) and cost 4 % in sustained runs of long launches
 //    (config 4, 270 steps: 129.1 -> 124.0 Gcell-updates/s at the power cap);
 //  * pacing cuts the DRAM traffic of cold bursts at full clocks (config 5: 1.19 -> 1.03 x
-//    algorithmic, 112 -> 137 Gcell-updates/s) but costs 8 % in sustained runs on every config
-//    (config 5: 131.3 -> 120.4), the regime a solver lives in: off unless asked for.
-constexpr int ps_pdl_max_steps = 96;      // dependent launches up to this many steps per CTA
+//    algorithmic, 108 -> 134 Gcell-updates/s; config 4: 130 -> 136) and, with the counter updated
+//    once per four stages, is neutral in sustained runs of long launches (config 4: 130.6 ->
+//    131.1, config 5: 131.3 -> 132.8); on short launches it costs 1-2 % (config 3) to 10 %
+//    (config 2).
+// So: short launches (up to ps_pdl_max_steps z steps per CTA) get dependent launches, long ones
+// get pacing.
+constexpr int ps_pdl_max_steps = 96;
 
 bool launch_dependent(const ps_ctx *c)
 {
@@ -158,7 +162,8 @@ bool launch_dependent(const ps_ctx *c)
 
 int launch_pace_window(const ps_ctx *c)
 {
-    return c->pace_mode >= 0 ? c->pace_mode : 0;
+    if (c->pace_mode >= 0) return c->pace_mode;
+    return c->fused.pace_steps > ps_pdl_max_steps ? ps::ZM_PACE_WINDOW : 0;
 }
 
 int resolve_variant(const ps_ctx *c, int req)
