@@ -306,7 +306,9 @@ int ps_ssf_rhs(ps_ctx *c, const double *F_dev, const double *kappa_dev, double s
  * all zero in the product build.  Synchronises the stream.
  * ps_debug_sabotage(c, 1) makes the checked kernel skip the red-barrier wait of its row warps (a
  * deliberately broken protocol, harmless to memory: the negative control of the checks);
- * PS_EINVAL in the product build. */
+ * ps_debug_sabotage(c, 2) makes CTA 0 of a paced launch never claim its stages in the pacing
+ * counter, as if it were not resident: the other CTAs must give up waiting (after ~1 ms each) and
+ * the launch must end with the right result.  PS_EINVAL in the product build. */
 int ps_checked_build(void);
 int ps_debug_read(ps_ctx *c, unsigned long long *out_host);
 int ps_debug_sabotage(ps_ctx *c, int mode);

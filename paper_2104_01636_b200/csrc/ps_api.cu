@@ -739,7 +739,7 @@ int ps_checked_build(void)
 
 int ps_debug_sabotage(ps_ctx *c, int mode)
 {
-    if (!c || mode < 0 || mode > 1) return PS_EINVAL;
+    if (!c || mode < 0 || mode > 2) return PS_EINVAL;
 #ifdef PS_CHECKED
     c->fused.sabotage = mode;
     return PS_OK;

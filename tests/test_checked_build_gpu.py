@@ -143,6 +143,37 @@ def test_checks_notice_a_broken_protocol(torch_cuda, B, checked):
         assert s.debug_read() == [0] * 8
 
 
+def test_pacing_gives_up_instead_of_deadlocking(torch_cuda, B, checked, ora):
+    """Pacing assumes that all CTAs of the persistent grid are resident at once.  If one of them
+    never shows up in the pacing counter (sabotage 2: CTA 0 does not claim its stages -- what a CTA
+    kept off the SMs by foreign work would look like) the others must not wait for ever: each gives
+    up after about a millisecond and runs free.  The launch ends, p is bitwise right, no ring
+    violation."""
+    import time
+    w = workload(128, 128, 64)                     # 18 tiles x 1 z chunk: 18 CTAs of 67 stages;
+                                                   # without CTA 0 the mean falls behind at stage 40
+    coef = ora.coefficients(w.F, w.rho_l, w.rho_g, w.dx, w.dy, w.dz)
+    p_ora = np.zeros_like(w.rhs)
+    ora.sweep(coef, w.rhs, p_ora, w.omega, 3)
+    with B.PoissonSolver(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, lib=checked) as s:
+        s.set_kernel(B.KERNEL_FUSED)
+        s.set_tuning(1, 1)
+        assert s.get_tuning()[3] == 18
+        s.set_launch_options(0, 2)
+        assert checked.ps_debug_sabotage(s._h, 2) == B.PS_OK
+        s.set_fraction(dev(torch_cuda, w.F), w.rho_l, w.rho_g)
+        rhs_d = dev(torch_cuda, w.rhs)
+        p_d = torch_cuda.zeros_like(rhs_d)
+        torch_cuda.cuda.synchronize()
+        t0 = time.perf_counter()
+        s.sweeps(rhs_d, p_d, w.omega, 3)
+        torch_cuda.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        assert 2e-3 < dt < 5.0, dt                   # 3 launches x (>= 1 ms of waiting + the sweep)
+        assert s.debug_read()[0] == 0, s.debug_read()
+        assert int(np.count_nonzero(p_d.cpu().numpy() != p_ora)) == 0
+
+
 # ------------------------------------------------------------------------------- guard bands
 GUARD = 4096          # doubles per guard zone (32 KB)
 
