@@ -7,7 +7,8 @@
 // global memory and on L2 round trips.  Here the whole problem lives on chip for the launch:
 //   * the launch is ONE cluster of C CTAs (C = 16, 8, 4, 2 or 1, the largest that divides nz);
 //     CTA r owns the z slab [r nz/C, (r+1) nz/C) and keeps p, ax, ay, rhs of the slab and az of
-//     the slab plus the plane below it in shared memory (loaded once, p written back once);
+//     the slab plus the plane below it in shared memory (loaded once, p written back once),
+//     each field colour-compacted (see cl_smem_bytes);
 //   * a half-sweep updates the cells of one colour in place in shared memory; the z neighbours
 //     of the slab's first and last plane are read from the neighbouring CTA's shared memory
 //     (distributed shared memory, periodic in the cluster rank).  Cells of one colour never read
@@ -25,11 +26,16 @@ constexpr int CL_THREADS = 1024;
 constexpr int CL_ITEMS = 3;            // x-pairs of cells per thread: a slab holds at most 6144 cells
 constexpr size_t CL_SMEM_MAX = 227 * 1024;
 
-// shared memory of one CTA: 4 slab fields (p, ax, ay, rhs) + az with one extra plane
+// Shared memory of one CTA.  Every field is stored COLOUR-COMPACTED: one array per colour, entry
+// ih + hx (j + ny kl) with hx = ceil(nx / 2) holding the cell of that colour in the x-pair ih of row
+// (j, kl).  A half-sweep then reads its own colour's entry and the other colour's neighbours at
+// unit stride across a warp (2 shared-memory wavefronts per 8-byte access instead of the 4 of a
+// natural layout read at stride 2, which made the shared-memory pipe the limit at 65 k cells).
+// 4 slab fields (p, ax, ay, rhs) + az with one extra plane below the slab, two colours each.
 inline size_t cl_smem_bytes(const Grid &g, int C)
 {
-    const size_t plane = (size_t)g.nx * g.ny, pz = (size_t)(g.nz / C);
-    return (4 * pz * plane + (pz + 1) * plane) * sizeof(double);
+    const size_t planec = (size_t)((g.nx + 1) / 2) * g.ny, pz = (size_t)(g.nz / C);
+    return 2 * (4 * pz * planec + (pz + 1) * planec) * sizeof(double);
 }
 
 // the cluster size for this grid, or 0 if it does not fit
@@ -54,74 +60,94 @@ ps_cluster_sweeps_kernel(Grid g, const double *__restrict__ ax, const double *__
     extern __shared__ __align__(16) double cl_smem[];
     const int C = (int)cluster.num_blocks(), rank = (int)cluster.block_rank();
     const int pz = g.nz / C, k0 = rank * pz;
-    const int plane = g.nx * g.ny, slab = pz * plane;
-    double *P = cl_smem, *AX = P + slab, *AY = AX + slab, *RH = AY + slab, *AZ = RH + slab;
-    // AZ: plane 0 = az of the plane below the slab (periodic), planes 1..pz = the slab's own
+    const int hx = (g.nx + 1) >> 1;
+    const int plane = g.nx * g.ny, slab = pz * plane;       // natural layout (global memory)
+    const int planec = hx * g.ny, slabc = pz * planec;      // one colour (shared memory)
+    // per colour c: P[c], AX[c], AY[c], RH[c] of slabc entries; AZ[c] of slabc + planec entries,
+    // its first plane = az of the plane below the slab (periodic)
+    // (addresses by arithmetic: arrays of pointers indexed by the colour would live in local memory)
+    auto fP = [&](int c) { return cl_smem + c * slabc; };
+    auto fAX = [&](int c) { return cl_smem + (2 + c) * slabc; };
+    auto fAY = [&](int c) { return cl_smem + (4 + c) * slabc; };
+    auto fRH = [&](int c) { return cl_smem + (6 + c) * slabc; };
+    auto fAZ = [&](int c) { return cl_smem + 8 * slabc + c * (slabc + planec); };
     const size_t base = (size_t)k0 * plane;
     for (int n = threadIdx.x; n < slab; n += CL_THREADS) {
-        P[n] = p[base + n];
-        AX[n] = ax[base + n];
-        AY[n] = ay[base + n];
-        RH[n] = rhs[base + n];
-        AZ[plane + n] = az[base + n];
+        const int i = n % g.nx, t = n / g.nx;
+        const int j = t % g.ny, kl = t / g.ny;
+        const int c = (i + j + k0 + kl) & 1, q = (i >> 1) + hx * (j + g.ny * kl);
+        fP(c)[q] = p[base + n];
+        fAX(c)[q] = ax[base + n];
+        fAY(c)[q] = ay[base + n];
+        fRH(c)[q] = rhs[base + n];
+        fAZ(c)[planec + q] = az[base + n];
     }
     const size_t below = (size_t)(k0 > 0 ? k0 - 1 : g.nz - 1) * plane;
-    for (int n = threadIdx.x; n < plane; n += CL_THREADS) AZ[n] = az[below + n];
+    for (int n = threadIdx.x; n < plane; n += CL_THREADS) {
+        const int i = n % g.nx, j = n / g.nx;
+        fAZ((i + j + k0 + 1) & 1)[(i >> 1) + hx * j] = az[below + n];     // plane k0 - 1
+    }
     // the slabs of the z neighbours (the CTA itself when the cluster is one CTA: periodic)
-    const double *Pdn = cluster.map_shared_rank(P, rank > 0 ? rank - 1 : C - 1);
-    const double *Pup = cluster.map_shared_rank(P, rank + 1 < C ? rank + 1 : 0);
+    const int rdn = rank > 0 ? rank - 1 : C - 1, rup = rank + 1 < C ? rank + 1 : 0;
+    const double *Pdn0 = cluster.map_shared_rank(cl_smem, rdn);       // their P of colour 0
+    const double *Pup0 = cluster.map_shared_rank(cl_smem, rup);
     cluster.sync();
 
     // A thread keeps the same (at most CL_ITEMS) x-pairs of cells for the whole launch -- in each
     // half-sweep it updates the cell of the pair that has the active colour -- so everything that
-    // does not depend on the colour is worked out once, here: the index of the pair's left cell,
-    // which of its two cells is red, where its six neighbours are (clamped at the walls, where
-    // the coefficient is 0.0; the z neighbours of the slab's end planes in the neighbour CTA).
-    const int hx = (g.nx + 1) >> 1;
-    const int items = hx * g.ny * pz;
-    int n0[CL_ITEMS], m0[CL_ITEMS], par[CL_ITEMS], edge[CL_ITEMS];
+    // does not depend on the colour is worked out once, here.
+    const int items = slabc;
+    int m0[CL_ITEMS], par[CL_ITEMS], edge[CL_ITEMS];
 #pragma unroll
     for (int q = 0; q < CL_ITEMS; ++q) {
         const int h = (int)threadIdx.x + q * CL_THREADS;
-        n0[q] = -1;
-        m0[q] = par[q] = edge[q] = 0;
+        m0[q] = -1;
+        par[q] = edge[q] = 0;
         if (h < items) {
             const int ih = h % hx, t = h / hx;
             const int j = t % g.ny, kl = t / g.ny;
-            m0[q] = 2 * ih + g.nx * j;                            // index inside a plane
-            n0[q] = m0[q] + plane * kl;
-            par[q] = (j + k0 + kl) & 1;                           // the red cell of the pair: i = 2 ih + par
-            edge[q] = (2 * ih == 0 ? 1 : 0) | (2 * ih + 2 >= g.nx ? 2 : 0) | (j == 0 ? 4 : 0) |
-                      (j == g.ny - 1 ? 8 : 0) | (kl == 0 ? 16 : 0) | (kl == pz - 1 ? 32 : 0) |
-                      (2 * ih + 1 >= g.nx ? 64 : 0);              // odd nx: the pair has one cell
+            m0[q] = ih + hx * j;                                  // entry inside a plane
+            par[q] = (j + k0 + kl) & 1;                           // the pair's red cell: i = 2 ih + par
+            edge[q] = (ih == 0 ? 1 : 0) | (2 * ih == g.nx - 1 ? 2 : 0) | (2 * ih + 1 == g.nx - 1 ? 128 : 0) |
+                      (j == 0 ? 4 : 0) | (j == g.ny - 1 ? 8 : 0) | (kl == 0 ? 16 : 0) |
+                      (kl == pz - 1 ? 32 : 0) | (2 * ih + 1 >= g.nx ? 64 : 0);   // 64: odd nx, one cell
         }
     }
     for (int s = 0; s < 2 * nsweeps; ++s) {
-        const int colour = s & 1;
+        const int c = s & 1, o = c ^ 1;                           // active colour, the other colour
+        double *Pc = fP(c);
+        const double *Po = fP(o), *AXc = fAX(c), *AXo = fAX(o), *AYc = fAY(c), *AYo = fAY(o),
+                     *AZc = fAZ(c), *AZo = fAZ(o), *RHc = fRH(c);
+        const double *Pdn = Pdn0 + o * slabc, *Pup = Pup0 + o * slabc;
 #pragma unroll
         for (int q = 0; q < CL_ITEMS; ++q) {
-            if (n0[q] < 0) continue;
-            const int off = par[q] ^ colour;                      // 0: left cell, 1: right cell
+            if (m0[q] < 0) continue;
+            const int off = par[q] ^ c;                           // 0: left cell of the pair, 1: right
             const int e = edge[q];
             if (off && (e & 64)) continue;
-            const int n = n0[q] + off;
-            const bool wxm = (e & 1) && !off, wxp = (e & 2) && (off || (e & 64));
-            const int m = m0[q] + off;
-            const double axm = wxm ? 0.0 : AX[n - 1], axp = AX[n];
-            const double aym = (e & 4) ? 0.0 : AY[n - g.nx], ayp = AY[n];
-            const double azm = AZ[n], azp = AZ[n + plane];
-            const double pxm = P[wxm ? n : n - 1];
-            const double pxp = P[wxp ? n : n + 1];
-            const double pym = P[(e & 4) ? n : n - g.nx];
-            const double pyp = P[(e & 8) ? n : n + g.nx];
-            const double pzm = (e & 16) ? Pdn[(pz - 1) * plane + m] : P[n - plane];
-            const double pzp = (e & 32) ? Pup[m] : P[n + plane];
-            P[n] = sor_update(axm, axp, aym, ayp, azm, azp, pxm, pxp, pym, pyp, pzm, pzp, P[n],
-                              RH[n], omega);
+            const int n = (int)threadIdx.x + q * CL_THREADS;      // entry in the colour arrays
+            const bool wxm = (e & 1) && !off;                     // the cell is at the x- / x+ wall
+            const bool wxp = off ? (e & 128) != 0 : (e & 2) != 0;
+            const double pc = Pc[n];
+            const double axm = wxm ? 0.0 : AXo[n - 1 + off], axp = AXc[n];
+            const double aym = (e & 4) ? 0.0 : AYo[n - hx], ayp = AYc[n];
+            const double azm = AZo[n], azp = AZc[n + planec];
+            const double pxm = wxm ? pc : Po[n - 1 + off];
+            const double pxp = wxp ? pc : Po[n + off];
+            const double pym = (e & 4) ? pc : Po[n - hx];
+            const double pyp = (e & 8) ? pc : Po[n + hx];
+            const double pzm = (e & 16) ? Pdn[(pz - 1) * planec + m0[q]] : Po[n - planec];
+            const double pzp = (e & 32) ? Pup[m0[q]] : Po[n + planec];
+            Pc[n] = sor_update(axm, axp, aym, ayp, azm, azp, pxm, pxp, pym, pyp, pzm, pzp, pc,
+                               RHc[n], omega);
         }
         cluster.sync();      // the colour just written is read by everybody in the next half-sweep
     }
-    for (int n = threadIdx.x; n < slab; n += CL_THREADS) p[base + n] = P[n];
+    for (int n = threadIdx.x; n < slab; n += CL_THREADS) {
+        const int i = n % g.nx, t = n / g.nx;
+        const int j = t % g.ny, kl = t / g.ny;
+        p[base + n] = fP((i + j + k0 + kl) & 1)[(i >> 1) + hx * (j + g.ny * kl)];
+    }
 }
 
 // One-time set-up of the kernel's attributes; returns the cluster size this device can run for
@@ -137,8 +163,7 @@ inline int cl_plan(const Grid &g)
         cudaGetLastError();
         return 0;
     }
-    cudaLaunchConfig_t cfg;
-    memset(&cfg, 0, sizeof cfg);
+    cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)C);
     cfg.blockDim = dim3(CL_THREADS);
     cfg.dynamicSmemBytes = cl_smem_bytes(g, C);
@@ -162,8 +187,7 @@ inline cudaError_t cl_launch(const Grid &g, int C, const double *ax, const doubl
                              const double *az, const double *rhs, double *p, double omega,
                              int nsweeps, cudaStream_t stream)
 {
-    cudaLaunchConfig_t cfg;
-    memset(&cfg, 0, sizeof cfg);
+    cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)C);
     cfg.blockDim = dim3(CL_THREADS);
     cfg.dynamicSmemBytes = cl_smem_bytes(g, C);
