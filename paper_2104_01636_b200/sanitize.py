@@ -2,6 +2,7 @@
 
     python -m paper_2104_01636_b200.sanitize [--md FILE] [--tools memcheck,initcheck,racecheck,synccheck]
     python -m paper_2104_01636_b200.sanitize --target        (what the tools run; also fine alone)
+    python -m paper_2104_01636_b200.sanitize --soak          (long-run repeatability, see soak())
 
 The target drives every kernel family through the C ABI on two small grids -- BASELINE.json's
 config 1 (32x32x64, one bubble) and a ragged multi-tile grid (186x46x8 with a random F in
@@ -117,15 +118,54 @@ def summarise(tool, cmd, rc, secs, out) -> str:
     return "\n".join(head)
 
 
+def soak(runs=((3, 20000), (4, 4000), (5, 800))) -> int:
+    """Long-run repeatability of the hand-synchronised fused sweep: n sweeps on each config with
+    the library's launch options, free running, dependent launches + pacing window 1, and the
+    library's options again -- all four fields must be bitwise equal and finite (a rare miss in
+    the mbarrier protocol, the pacing or the grid-dependency wait would show up as a difference).
+    Prints one JSON line per run; returns the number of runs that differed."""
+    import json
+    import torch
+    from . import binding as B, build, workload as wl
+    build.build()
+    B.load()
+    assert torch.cuda.is_available(), "sanitize --soak needs the GPU"
+    bad = 0
+    for cfg, n in runs:
+        w = wl.make_config(cfg)
+        F = torch.from_numpy(w.F).cuda()
+        rhs = torch.from_numpy(w.rhs).cuda()
+        ref = None
+        for dep, window in ((-1, -1), (0, 0), (1, 1), (-1, -1)):
+            with B.PoissonSolver(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz) as s:
+                s.set_kernel(B.KERNEL_FUSED)
+                s.set_launch_options(dep, window)
+                s.set_fraction(F, w.rho_l, w.rho_g)
+                p = torch.zeros_like(rhs)
+                s.sweeps(rhs, p, w.omega, n)
+                torch.cuda.synchronize()
+                if ref is None:
+                    ref = p.clone()
+                ok = bool(torch.equal(p, ref)) and bool(torch.isfinite(p).all())
+                bad += 0 if ok else 1
+                print(json.dumps({"config": cfg, "sweeps": n, "dependent_launch, pace_window":
+                                  s.get_launch_options(), "bitwise_equal_and_finite": ok}), flush=True)
+        del ref
+    return bad
+
+
 def main(argv=None) -> int:
     ap = argparse.ArgumentParser()
     ap.add_argument("--target", action="store_true")
+    ap.add_argument("--soak", action="store_true")
     ap.add_argument("--tools", default="memcheck,initcheck,racecheck,synccheck")
     ap.add_argument("--timeout", type=int, default=1500, help="seconds per tool")
     ap.add_argument("--md", default="")
     args = ap.parse_args(argv)
     if args.target:
         return target()
+    if args.soak:
+        return 1 if soak() else 0
     parts = []
     for tool in args.tools.split(","):
         parts.append(summarise(tool, *run_tool(tool, args.timeout)))
