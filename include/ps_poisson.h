@@ -217,8 +217,9 @@ int ps_timing(ps_ctx *c, double *sweep_ms, long long *sweep_launches, long long 
  * 1/16 of the sum of the 4 fine face coefficients on the coarse face; restriction = mean of the
  * 8 children of r = rhs - A p; piecewise-constant prolongation added to p; red-black SOR
  * (omega_s on the finest level, omega_c on every coarser one) as smoother (nu1 before, nu2
- * after; on level l multiplied by nu_growth^l up to nu_max, because coarse levels are cheap and
- * the bubble modes need them solved accurately) and as coarsest-level solver (coarse_sweeps);
+ * after; on level l multiplied by nu_growth^l up to nu_max -- min(nu_max, nu_max_deep) from
+ * level 2 on --, because coarse levels are cheap and the bubble modes need level 1 solved
+ * accurately) and as coarsest-level solver (coarse_sweeps);
  * gamma = 1 (V cycle) or 2 (W cycle). */
 typedef struct {
     int levels;          /* requested levels, clipped to [1, what the grid allows]            */
@@ -230,6 +231,8 @@ typedef struct {
     double omega_s;      /* relaxation factor of every sweep on level 0, in (0,2)              */
     double omega_c;      /* relaxation factor of every sweep on the levels l >= 1 (smoother    */
                          /* and coarsest solver), in (0,2)                                     */
+    int nu_max_deep;     /* cap of the per-level count on the levels l >= 2 (>= 1; level 1 is  */
+                         /* capped by nu_max alone; values >= nu_max change nothing)           */
 } ps_mg_params;
 
 /* Device memory of the coarse levels (per level: coefficients, ping-pong buffer, reduction

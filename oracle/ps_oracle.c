@@ -278,13 +278,18 @@ typedef struct {
  * residual, restriction to the rhs of level l+1, zero initial guess there, gamma recursive
  * cycles (1 = V, 2 = W), prolongation added to p, nu2 sweeps.  On level l the smoothing counts are
  * min(nu * nu_growth^l, nu_max) (never below nu): coarse levels are cheap and the bubble modes
- * need them solved accurately (DESIGN.md §12 M6).  Every sweep of level 0 uses omega_s, every
+ * need them solved accurately (DESIGN.md §12 M6); from level 2 on the cap is
+ * min(nu_max, nu_max_deep).  Every sweep of level 0 uses omega_s, every
  * sweep of a level l >= 1 (smoothing and the coarsest solve) omega_c. */
 static int mg_nu(int nu, int l, const ora_mg_params *prm)
 {
+    /* the cap of level l: nu_max on level 1, min(nu_max, nu_max_deep) from level 2 on (the
+     * bubble-offset modes are representable down to level 1 only: that is where
+     * the sweeps pay; the levels below need fewer) */
+    const int cap = (l >= 2 && prm->nu_max_deep < prm->nu_max) ? prm->nu_max_deep : prm->nu_max;
     long long v = nu;
-    for (int q = 0; q < l && v < prm->nu_max; ++q) v *= prm->nu_growth;
-    return (int)(v < prm->nu_max ? v : (nu < prm->nu_max ? prm->nu_max : nu));
+    for (int q = 0; q < l && v < cap; ++q) v *= prm->nu_growth;
+    return (int)(v < cap ? v : (nu < cap ? cap : nu));
 }
 
 static void mg_cycle(mg_level *lv, int l, int nlev, const ora_mg_params *prm)

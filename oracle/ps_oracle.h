@@ -43,6 +43,8 @@ typedef struct {
                           * levels = 1) */
     double omega_c;      /* relaxation factor on the coarse levels l >= 1: smoother and coarsest
                           * solver (DESIGN.md §12 M6) */
+    int nu_max_deep;     /* cap of the per-level smoothing count on the levels l >= 2 (level 1 is
+                          * capped by nu_max alone); values >= nu_max change nothing */
 } ora_mg_params;
 
 void ora_mg_coarsen(int nx, int ny, int nz, const double *ax, const double *ay, const double *az,

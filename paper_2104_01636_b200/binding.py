@@ -30,7 +30,7 @@ KERNEL_NAMES = {KERNEL_AUTO: "auto", KERNEL_TWOPASS: "twopass", KERNEL_FUSED: "f
 # not on all.  The one place they are written down: bench.py, report.py and the parity tests take
 # them from here.
 MG_DEFAULTS = dict(levels=6, nu1=0, nu2=2, coarse_sweeps=10, gamma=1, omega_s=1.4, omega_c=1.97,
-                   nu_growth=24, nu_max=48)
+                   nu_growth=24, nu_max=48, nu_max_deep=48)
 
 # every symbol include/ps_poisson.h declares (tests check the library exports each one)
 SYMBOLS = ("ps_create", "ps_destroy", "ps_workspace_bytes", "ps_set_workspace", "ps_set_stream",
@@ -55,7 +55,8 @@ class _MgParams(ctypes.Structure):
     _fields_ = [("levels", ctypes.c_int), ("nu1", ctypes.c_int), ("nu2", ctypes.c_int),
                 ("nu_growth", ctypes.c_int), ("nu_max", ctypes.c_int),
                 ("coarse_sweeps", ctypes.c_int), ("gamma", ctypes.c_int),
-                ("omega_s", ctypes.c_double), ("omega_c", ctypes.c_double)]
+                ("omega_s", ctypes.c_double), ("omega_c", ctypes.c_double),
+                ("nu_max_deep", ctypes.c_int)]
 
 
 class _Info(ctypes.Structure):
@@ -330,21 +331,27 @@ class PoissonSolver:
     def mg_setup(self, levels: int | None = None, nu1: int | None = None, nu2: int | None = None,
                  coarse_sweeps: int | None = None, gamma: int | None = None,
                  omega_s: float | None = None, nu_growth: int | None = None,
-                 nu_max: int | None = None, omega_c: float | None = None) -> int:
+                 nu_max: int | None = None, omega_c: float | None = None,
+                 nu_max_deep: int | None = None) -> int:
         """Build the level hierarchy from the current coefficients; returns the levels in use.
         With no arguments: MG_DEFAULTS.  Any argument given replaces its default, except that
         omega_c follows an explicitly given omega_s when it is not given itself (one relaxation
-        factor on every level)."""
+        factor on every level), and nu_max_deep an explicitly given nu_max (one cap on every
+        level)."""
         self._sync_stream()
         if omega_c is None and omega_s is not None:
             omega_c = omega_s
+        if nu_max_deep is None and nu_max is not None:
+            nu_max_deep = nu_max
         given = dict(levels=levels, nu1=nu1, nu2=nu2, coarse_sweeps=coarse_sweeps, gamma=gamma,
-                     omega_s=omega_s, omega_c=omega_c, nu_growth=nu_growth, nu_max=nu_max)
+                     omega_s=omega_s, omega_c=omega_c, nu_growth=nu_growth, nu_max=nu_max,
+                     nu_max_deep=nu_max_deep)
         q = dict(MG_DEFAULTS)
         q.update({k: v for k, v in given.items() if v is not None})
         levels = q["levels"]
         prm = _MgParams(q["levels"], q["nu1"], q["nu2"], q["nu_growth"], q["nu_max"],
-                        q["coarse_sweeps"], q["gamma"], q["omega_s"], q["omega_c"])
+                        q["coarse_sweeps"], q["gamma"], q["omega_s"], q["omega_c"],
+                        q["nu_max_deep"])
         if self._torch_owns:               # the level memory is a torch allocation too
             need = self._lib.ps_mg_workspace_bytes(self._h, levels)
             if need and (self._mg_ws is None or self._mg_ws[0].numel() < need + 256):

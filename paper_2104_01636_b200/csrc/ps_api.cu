@@ -874,9 +874,10 @@ int mg_launch_prolong_add(ps_ctx *f, const double *ec, double *p)
 
 int mg_nu(int nu, int level, const ps_mg_params &m)
 {
+    const int cap = (level >= 2 && m.nu_max_deep < m.nu_max) ? m.nu_max_deep : m.nu_max;
     long long v = nu;
-    for (int q = 0; q < level && v < m.nu_max; ++q) v *= m.nu_growth;
-    return (int)(v < m.nu_max ? v : (nu < m.nu_max ? m.nu_max : nu));
+    for (int q = 0; q < level && v < cap; ++q) v *= m.nu_growth;
+    return (int)(v < cap ? v : (nu < cap ? cap : nu));
 }
 
 // The finest level of ps_mg_solve may take its norm inside the residual + restriction pass: with
@@ -951,6 +952,7 @@ int ps_mg_setup(ps_ctx *c, const ps_mg_params *prm)
 {
     if (!c || !prm) return PS_EINVAL;
     if (prm->nu1 < 0 || prm->nu2 < 0 || prm->nu_growth < 1 || prm->nu_max < 1 ||
+        prm->nu_max_deep < 1 ||
         prm->coarse_sweeps < 1 || prm->gamma < 1 ||
         prm->gamma > 2 || !(prm->omega_s > 0.0 && prm->omega_s < 2.0) ||
         !(prm->omega_c > 0.0 && prm->omega_c < 2.0))

@@ -2,7 +2,7 @@
 
     python -m paper_2104_01636_b200.mg_tune --configs 3,4 --omega-s 1.4,1.5,1.6 \
         --omega-c 1.9,1.95 --nu-growth 4,16 --nu-max 16,32 [--nu 0:2,1:1] [--coarse-sweeps 10,30] \
-        [--levels 6] [--gamma 1] [--max-cycles 400] [--seed-offset 0] [--md FILE]
+        [--nu-max-deep 0] [--levels 6] [--gamma 1] [--max-cycles 400] [--seed-offset 0] [--md FILE]
 
 Every combination of the listed values is run through `ps_mg_setup` + `ps_mg_solve(tol = 1e-8)`
 from p = 0 (after one untimed warm-up solve per config, so that level memory and kernels are
@@ -39,6 +39,7 @@ def main(argv=None):
     ap.add_argument("--omega-c", default="1.95")
     ap.add_argument("--nu-growth", default="16")
     ap.add_argument("--nu-max", default="32")
+    ap.add_argument("--nu-max-deep", default="0", help="cap from level 2 on (0 = nu_max)")
     ap.add_argument("--max-cycles", type=int, default=400)
     ap.add_argument("--seed-offset", type=int, default=0,
                     help="another bubble arrangement and rhs of the same recipe (workload.make_config)")
@@ -54,7 +55,7 @@ def main(argv=None):
     nus = [tuple(int(v) for v in q.split(":")) for q in args.nu.split(",")]
     grid = list(itertools.product(_ints(args.levels), nus, _ints(args.coarse_sweeps),
                                   _ints(args.gamma), _floats(args.omega_s), _floats(args.omega_c),
-                                  _ints(args.nu_growth), _ints(args.nu_max)))
+                                  _ints(args.nu_growth), _ints(args.nu_max), _ints(args.nu_max_deep)))
     results = {}
     for cfg in cfgs:
         w = wl.make_config(cfg, seed_offset=args.seed_offset)
@@ -65,9 +66,9 @@ def main(argv=None):
             s.set_fraction(F_d, w.rho_l, w.rho_g)
             s.mg_setup()
             s.mg_solve(rhs_d, p_d, 2, 0.0)
-            for lv, (nu1, nu2), cs, gm, os_, oc, g, m in grid:
+            for lv, (nu1, nu2), cs, gm, os_, oc, g, m, md in grid:
                 prm = dict(levels=lv, nu1=nu1, nu2=nu2, coarse_sweeps=cs, gamma=gm, omega_s=os_,
-                           omega_c=oc, nu_growth=g, nu_max=m)
+                           omega_c=oc, nu_growth=g, nu_max=m, nu_max_deep=md or m)
                 p_d.zero_()
                 torch.cuda.synchronize()
                 t0 = time.perf_counter()
@@ -81,8 +82,8 @@ def main(argv=None):
                 results.setdefault(tuple(prm.items()), {})[cfg] = rec
     rows = sorted(results.items(),
                   key=lambda kv: kv[1][cfgs[-1]]["seconds"] if kv[1][cfgs[-1]]["converged"] else 1e9)
-    head = ("| levels | V(nu1,nu2) | coarsest | gamma | omega_s | omega_c | growth | nu_max | "
-            + " | ".join(f"cfg {c}: cycles | s" for c in cfgs) + " |\n|" + "---|" * (8 + 2 * len(cfgs)) + "\n")
+    head = ("| levels | V(nu1,nu2) | coarsest | gamma | omega_s | omega_c | growth | nu_max | deep | "
+            + " | ".join(f"cfg {c}: cycles | s" for c in cfgs) + " |\n|" + "---|" * (9 + 2 * len(cfgs)) + "\n")
     body = ""
     for key, per in rows:
         q = dict(key)
@@ -90,7 +91,8 @@ def main(argv=None):
             (f"{per[c]['cycles']} | {per[c]['seconds']:.4f}" if per[c]["converged"]
              else f"not converged ({per[c]['res_rel']:.1e}) | -") for c in cfgs)
         body += (f"| {q['levels']} | V({q['nu1']},{q['nu2']}) | {q['coarse_sweeps']} | {q['gamma']} | "
-                 f"{q['omega_s']} | {q['omega_c']} | {q['nu_growth']} | {q['nu_max']} | {cells} |\n")
+                 f"{q['omega_s']} | {q['omega_c']} | {q['nu_growth']} | {q['nu_max']} | "
+                 f"{q['nu_max_deep']} | {cells} |\n")
     md = head + body
     print(md)
     if args.md:

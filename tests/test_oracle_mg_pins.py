@@ -262,3 +262,51 @@ def test_binding_defaults_converge_in_tens_of_cycles_in_the_oracle(ora):
     assert all(b < a for a, b in zip(res[2:], res[3:]))
     r = w.rhs - ora.apply(coef, p)
     assert np.linalg.norm(r) <= 1.0001e-8 * np.linalg.norm(w.rhs)
+
+
+def _cycle_by_hand(ora, coefs, l, rhs, p, post, coarse, w0, wc):
+    """M6 spelled out from the oracle's step functions, V(0, post[l]) with an explicit list of
+    post-smoothing counts per level (the schedule is what the test states, not a formula)."""
+    w = w0 if l == 0 else wc
+    if l == len(coefs) - 1:
+        ora.sweep(coefs[l], rhs, p, w, coarse)
+        return
+    rc = ora.mg_restrict(ora.mg_residual_field(coefs[l], rhs, p))
+    e = np.zeros_like(rc)
+    _cycle_by_hand(ora, coefs, l + 1, rc, e, post, coarse, w0, wc)
+    ora.mg_prolong_add(e, p)
+    ora.sweep(coefs[l], rhs, p, w, post[l])
+
+
+def test_deep_levels_have_their_own_cap(ora):
+    """M6: the smoothing count of level l is min(nu g^l, nu_max) on level 1 and
+    min(nu g^l, nu_max, nu_max_deep) from level 2 on.  Five levels on 32 x 32 x 64 with nu = 2,
+    g = 3, nu_max = 7, nu_max_deep = 4: counts 2, 6, 4, 4 and 5 coarsest sweeps -- against the cycle
+    assembled by hand from the oracle's steps with that list; nu_max_deep >= nu_max changes
+    nothing; a cap that also bound level 1 (or none at all) gives another result."""
+    nx, ny, nz = 32, 32, 64
+    assert ora.mg_max_levels(nx, ny, nz) >= 5
+    coef = var_coef(ora, nx, ny, nz, 61)
+    rhs = wl.remove_mean(rnd((nz, ny, nx), 62))
+    kw = dict(levels=5, nu1=0, nu2=2, coarse_sweeps=5, omega_s=1.3, omega_c=1.8, nu_growth=3, nu_max=7)
+    coefs = [coef]
+    for _ in range(4):
+        coefs.append(ora.mg_coarsen(coefs[-1]))
+    p = np.zeros_like(rhs)
+    ora.mg_solve(coef, rhs, p, 2, 0.0, nu_max_deep=4, **kw)
+    q = np.zeros_like(rhs)
+    for _ in range(2):
+        _cycle_by_hand(ora, coefs, 0, rhs, q, [2, 6, 4, 4], 5, 1.3, 1.8)
+    assert np.array_equal(p, q)
+    a, b, c = np.zeros_like(rhs), np.zeros_like(rhs), np.zeros_like(rhs)
+    ora.mg_solve(coef, rhs, a, 2, 0.0, **kw)                          # no deep cap: 2, 6, 7, 7
+    ora.mg_solve(coef, rhs, b, 2, 0.0, nu_max_deep=7, **kw)
+    ora.mg_solve(coef, rhs, c, 2, 0.0, nu_max_deep=99, **kw)
+    assert np.array_equal(a, b) and np.array_equal(a, c) and not np.array_equal(a, p)
+    r = np.zeros_like(rhs)
+    for _ in range(2):
+        _cycle_by_hand(ora, coefs, 0, rhs, r, [2, 6, 7, 7], 5, 1.3, 1.8)
+    assert np.array_equal(a, r)
+    d = np.zeros_like(rhs)
+    ora.mg_solve(coef, rhs, d, 2, 0.0, **dict(kw, nu_max=4))          # 2, 4, 4, 4: level 1 bound too
+    assert not np.array_equal(d, p)

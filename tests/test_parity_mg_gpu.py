@@ -92,6 +92,7 @@ PARAMS = [
     dict(levels=99, nu1=2, nu2=1, coarse_sweeps=40, gamma=1, omega_s=1.6, nu_growth=4, nu_max=16),
     dict(levels=99, nu1=0, nu2=2, coarse_sweeps=30, gamma=1, omega_s=1.75, nu_growth=4, nu_max=16),  # round 1's defaults
     dict(levels=99, nu1=1, nu2=2, coarse_sweeps=9, gamma=1, omega_s=1.45, omega_c=1.9, nu_growth=3, nu_max=12),  # two relaxation factors
+    dict(levels=99, nu1=0, nu2=2, coarse_sweeps=6, gamma=1, omega_s=1.4, omega_c=1.9, nu_growth=8, nu_max=16, nu_max_deep=5),  # fewer sweeps below level 1
     None,                                                                                             # binding.MG_DEFAULTS
 ]
 
@@ -240,7 +241,8 @@ def test_level_memory_is_caller_owned_and_setup_failures_leave_no_half_built_hie
         assert lib.ps_mg_set_workspace(s._h, ctypes.c_void_p(base + 8), need) == B.PS_EINVAL   # misaligned
         assert lib.ps_mg_set_workspace(s._h, ctypes.c_void_p(base), need // 2) == B.PS_OK
         c_prm = B._MgParams(prm["levels"], prm["nu1"], prm["nu2"], prm["nu_growth"], prm["nu_max"],
-                            prm["coarse_sweeps"], prm["gamma"], prm["omega_s"], prm["omega_s"])
+                            prm["coarse_sweeps"], prm["gamma"], prm["omega_s"], prm["omega_s"],
+                            prm["nu_max"])
         assert lib.ps_mg_setup(s._h, ctypes.byref(c_prm)) == B.PS_EINVAL
         assert lib.ps_mg_levels(s._h) == 0
         rhs_d = dev(torch_cuda, w.rhs)
