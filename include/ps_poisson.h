@@ -112,9 +112,11 @@ int ps_get_kernel(const ps_ctx *c);          /* the variant AUTO resolved to, or
 /* Launch geometry of the fused kernel (tuning and tests; every setting gives bitwise identical p).
  * rows_per_thread: rows of the 64x16-cell box one thread updates per step; only 1 (16 row warps)
  * is built -- two rows per thread were measured slower on B200 throughout round 1 -- so 0 (keep)
- * and 1 are accepted.  z_chunks: 0 = the balanced split (the (tile, plane) pairs of the grid cut
- * into one contiguous range per CTA, every CTA marching the same number of planes); n > 0 = every
- * (x,y) tile cut into n z chunks, the tile x chunk items dealt round-robin to the CTAs.
+ * and 1 are accepted.  z_chunks: 0 = the balanced split (the chunk count whose slowest CTA marches
+ * the fewest planes; the items left over after the last full round of one item per SM are cut
+ * again into equal z pieces, so that every CTA marches nearly the same number of planes);
+ * n > 0 = every (x,y) tile cut into n z chunks, the tile x chunk items dealt round-robin to
+ * the CTAs, no re-cut.
  * Synchronises the stream.  PS_EINVAL: fused kernel not available for this grid, values out of
  * range.  ps_get_tuning returns the setting, the number of tiles, of CTAs launched and of work
  * items (any output may be NULL). */
