@@ -570,3 +570,36 @@ def test_odd_check_interval_needs_no_copy_and_matches_oracle(torch_cuda, B, ora)
                 assert_p_parity(p_d.cpu().numpy(), p_ora, f"K={K} kernel {kernel}")
                 assert abs(ig.res_rel - io.res_rel) <= NORM_TOL * io.res_rel
                 assert s.residual(rhs_d, p_d)[1] == ig.res_rel    # p_dev holds what was measured
+
+
+EDGE_SHAPES = [(64, 1, 8), (2, 1, 2), (66, 2, 4), (130, 1, 6), (4, 5, 256), (256, 3, 2), (62, 15, 4),
+               (64, 16, 2), (128, 14, 2), (70, 29, 6), (2, 2, 2), (6, 1, 4), (68, 30, 12), (192, 17, 8)]
+
+
+@pytest.mark.parametrize("shape", EDGE_SHAPES)
+def test_edge_shapes_all_variants_and_default_multigrid(torch_cuda, B, ora, shape):
+    """Degenerate and boundary shapes of the tilings: one row, one pair, exactly one box of rows,
+    one row more or fewer than a tile, one column pair more than a tile, the smallest nz, a long
+    thin duct -- every kernel variant the library accepts, 1 and 3 sweeps, and two default
+    multigrid cycles (as many levels as the shape allows), all bitwise against the oracle."""
+    nx, ny, nz = shape
+    w = shape_workload(nx, ny, nz, 0, 0, None, seed=5)
+    coef = ora.coefficients(w.F, w.rho_l, w.rho_g, w.dx, w.dy, w.dz)
+    F_d, rhs_d = to_dev(torch_cuda, w.F), to_dev(torch_cuda, w.rhs)
+    for nsweeps in (1, 3):
+        p_ora = np.zeros_like(w.rhs)
+        ora.sweep(coef, w.rhs, p_ora, w.omega, nsweeps)
+        for variant in variants_for(B, w, tunings=((1, 0, -1, -1), (1, 1, 1, 2), (1, 2, 0, 0))):
+            with make_solver(B, w, variant) as s:
+                s.set_fraction(F_d, w.rho_l, w.rho_g)
+                p_d = torch_cuda.zeros_like(rhs_d)
+                s.sweeps(rhs_d, p_d, w.omega, nsweeps)
+                assert_p_parity(p_d.cpu().numpy(), p_ora, f"{shape} variant {variant} x{nsweeps}")
+    q_ora = np.zeros_like(w.rhs)
+    ora.mg_solve(coef, w.rhs, q_ora, 2, 0.0, **B.MG_DEFAULTS)
+    with make_solver(B, w) as s:
+        s.set_fraction(F_d, w.rho_l, w.rho_g)
+        s.mg_setup()
+        q_d = torch_cuda.zeros_like(rhs_d)
+        s.mg_solve(rhs_d, q_d, 2, 0.0)
+        assert_p_parity(q_d.cpu().numpy(), q_ora, f"{shape} default multigrid")
