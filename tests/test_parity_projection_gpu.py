@@ -41,7 +41,10 @@ def same(got, want, what):
 
 
 SHAPES = [(16, 12, 20, (0.1, 0.07, 0.13)), (1, 1, 8, None), (5, 7, 6, None), (2, 3, 2, None),
-          (72, 52, 34, (1 / 72, 1 / 60, 1 / 50)), (132, 20, 10, None)]
+          (72, 52, 34, (1 / 72, 1 / 60, 1 / 50)), (132, 20, 10, None),
+          # boundary shapes of the z-marching tiles (64 cells x 8 rows, z chunks of >= 4 planes)
+          (64, 1, 8, None), (66, 2, 4, None), (2, 1, 2, None), (130, 9, 6, None), (256, 3, 2, None),
+          (62, 15, 4, None), (64, 8, 40, None), (4, 5, 256, None)]
 
 
 @pytest.mark.parametrize("shape", SHAPES)
