@@ -46,6 +46,7 @@ extern "C" {
 #define PS_ESTATE  (-2)   /* call order: solve/residual/sweeps before ps_set_fraction      */
 #define PS_ECUDA   (-3)   /* a CUDA runtime call failed; ps_strerror gives the CUDA string */
 #define PS_ENOMEM  (-4)   /* host or device allocation failed                              */
+#define PS_ETOOBIG (-5)   /* ps_residual_noalloc: grid beyond PS_NOALLOC_MAX_CELLS           */
 
 /* Sweep kernel variants (ps_set_kernel).  All give bitwise identical p. */
 #define PS_KERNEL_AUTO     0   /* fastest variant the grid shape allows                     */
@@ -190,6 +191,47 @@ int ps_half_sweep(ps_ctx *c, const double *rhs_dev, double *p_dev, double omega,
  * Synchronises the stream.  Outputs are host pointers; res_rel / rhs_norm may be NULL. */
 int ps_residual(ps_ctx *c, const double *rhs_dev, const double *p_dev, double *res_abs,
                 double *res_rel, double *rhs_norm);
+
+/* ps_residual for callers that cannot allocate device memory.
+ *
+ * Who that is: this solver is meant to sit inside a flow solver's time step, and
+ * the residual of step 11 is evaluated in every one of them.  Such a host program
+ * usually hands the whole GPU to a memory pool of its own (a framework's caching allocator, an
+ * arena sized at start-up to the 180 GB of the board).  Inside it a cudaMalloc may simply fail
+ * because the pool already holds the memory, and cudaMalloc / cudaFree stall every stream of the
+ * device while they run, which a time step that overlaps several streams cannot afford.  A plug-in
+ * that is handed raw pointers and a stream, but no allocator, is in the same position.  Every other
+ * entry point of this header needs a ps_ctx, and ps_create allocates (host memory, a pinned
+ * read-back word, the fused kernel's plan); this one needs none.
+ *
+ * What it computes: out_dev[0] = ||rhs - A p||_2, out_dev[1] = that over ||rhs||_2 (the norm itself
+ * if rhs == 0), out_dev[2] = ||rhs||_2, with A given by the caller's face coefficients (the
+ * arrays ps_export_coefficients writes, or the caller's own in the same layout: +x, +y, +z face of
+ * every cell, 0 on the +x / +y wall faces).  Same summation tree as ps_residual, so the three
+ * numbers are bitwise the same.  All pointers are device pointers owned by the caller, the five
+ * fields 16-byte aligned and nx*ny*nz doubles, out_dev 3 doubles, 8-byte aligned.  One memset node
+ * and one kernel launch on cuda_stream (a cudaStream_t passed as void*, NULL = the legacy default
+ * stream); the call does not synchronise, out_dev is valid once the stream has reached that point.
+ *
+ * Scratch: the per-chunk partial sums live in a fixed array inside the library image (1 MiB +
+ * 256 B of device memory on every GPU that loads the library, held until the process exits), so
+ * the call runs no cudaMalloc, cudaFree, cudaMallocHost or any other allocating routine.  The
+ * price is a size limit: grids of more than PS_NOALLOC_MAX_CELLS cells (2^28: every BASELINE.json
+ * config fits, the largest has 151 M) are refused with PS_ETOOBIG before anything is enqueued.
+ * The first call on a device looks up the array's device address (that device must be current,
+ * as for every later call on it); make that first call outside any stream capture.
+ * All calls on one device share the array, which keeps what the last call left in it.  The one
+ * word that must start at zero (the counter by which the last block to finish is found) is
+ * cleared at the start of every call; the partial sums need no clearing, a call reads only the
+ * slots it has just written.  Two calls that can overlap on the GPU (different streams without
+ * an event between them, or two host threads on one device) race on the array and give garbage:
+ * order them.
+ * PS_EINVAL: NULL or misaligned pointer; nx, ny < 1; nz < 2 or odd.  PS_ETOOBIG: see above.
+ * PS_ECUDA: a runtime call failed (no device, sticky error). */
+#define PS_NOALLOC_MAX_CELLS 268435456LL
+int ps_residual_noalloc(int nx, int ny, int nz, const double *ax_dev, const double *ay_dev,
+                        const double *az_dev, const double *rhs_dev, const double *p_dev,
+                        void *cuda_stream, double *out_dev);
 
 /* The whole path on HOST buffers (the end-to-end leg of bench.py): H2D of F and rhs and p,
  * ps_set_fraction, ps_solve, D2H of p.  The three device staging fields come from the caller's

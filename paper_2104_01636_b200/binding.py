@@ -16,6 +16,8 @@ from dataclasses import dataclass
 from . import build as _build
 
 PS_OK, PS_EINVAL, PS_ESTATE, PS_ECUDA, PS_ENOMEM = 0, -1, -2, -3, -4
+PS_ETOOBIG = -5
+NOALLOC_MAX_CELLS = 1 << 28      # PS_NOALLOC_MAX_CELLS of include/ps_poisson.h
 KERNEL_AUTO, KERNEL_TWOPASS, KERNEL_FUSED, KERNEL_RESIDENT, KERNEL_FUSED_OTF = 0, 1, 2, 3, 4
 KERNEL_CLUSTER = 5
 KERNEL_NAMES = {KERNEL_AUTO: "auto", KERNEL_TWOPASS: "twopass", KERNEL_FUSED: "fused",
@@ -42,7 +44,7 @@ SYMBOLS = ("ps_create", "ps_destroy", "ps_workspace_bytes", "ps_set_workspace", 
            "ps_checked_build", "ps_debug_read", "ps_debug_sabotage", "ps_timing", "ps_launch_count", "ps_strerror",
            "ps_mg_workspace_bytes", "ps_mg_set_workspace", "ps_mg_setup", "ps_mg_levels", "ps_mg_solve", "ps_mg_export_coarse",
            "ps_mg_residual_restrict", "ps_mg_prolong_add", "ps_rhs_from_velocity",
-           "ps_correct_velocity", "ps_face_divergence", "ps_ssf_rhs")
+           "ps_correct_velocity", "ps_face_divergence", "ps_ssf_rhs", "ps_residual_noalloc")
 
 
 class PsError(RuntimeError):
@@ -134,6 +136,7 @@ def load(path: str | None = None) -> ctypes.CDLL:
     lib.ps_correct_velocity.argtypes = [vp, vp, d, vp, vp, vp]
     lib.ps_face_divergence.argtypes = [vp, vp, vp, vp, vp, d, vp]
     lib.ps_ssf_rhs.argtypes = [vp, vp, vp, d, vp]
+    lib.ps_residual_noalloc.argtypes = [i, i, i, vp, vp, vp, vp, vp, vp, vp]
     lib.ps_strerror.argtypes = [i]
     lib.ps_strerror.restype = ctypes.c_char_p
     if path == _build.LIB:
@@ -168,6 +171,29 @@ def _host_ptr(a, shape, name):
             and tuple(a.shape) == tuple(shape)):
         raise TypeError(f"{name}: expected a C-contiguous float64 array of shape {tuple(shape)}")
     return ctypes.c_void_p(a.ctypes.data)
+
+
+def residual_noalloc(ax, ay, az, rhs, p, out, lib=None):
+    """ps_residual_noalloc: the three numbers of `PoissonSolver.residual` written to the caller's
+    device tensor `out` (3 float64: ||r||, ||r||/||rhs||, ||rhs||), with the reduction's scratch
+    taken from a fixed array inside the library instead of a context's workspace.  For callers
+    that must not allocate device memory in the call -- a flow solver whose memory pool already
+    owns the board, where a cudaMalloc can fail or stalls every stream of the device.  Neither
+    this wrapper nor the library allocates: `out` is the caller's.  Enqueued on torch's current
+    stream, not synchronised; calls that may overlap on one GPU must be ordered by the caller (they
+    share the array).  Grids above NOALLOC_MAX_CELLS raise PsError(PS_ETOOBIG)."""
+    import torch
+    lib = lib if lib is not None else load()
+    nz, ny, nx = rhs.shape
+    ptrs = [_dev_ptr(t, rhs.shape, n) for t, n in
+            ((ax, "ax"), (ay, "ay"), (az, "az"), (rhs, "rhs"), (p, "p"))]
+    if not (isinstance(out, torch.Tensor) and out.is_cuda and out.dtype == torch.float64
+            and out.is_contiguous() and out.numel() >= 3):
+        raise TypeError("out: expected a contiguous CUDA float64 tensor of at least 3 elements")
+    s = torch.cuda.current_stream().cuda_stream
+    _check(lib, lib.ps_residual_noalloc(nx, ny, nz, *ptrs, ctypes.c_void_p(s),
+                                        ctypes.c_void_p(out.data_ptr())))
+    return out
 
 
 def fused_plan(nx: int, ny: int, nz: int, sm_count: int = 148, z_chunks: int = 0):

@@ -3,6 +3,7 @@
 // arguments, carves the workspace and enqueues launches.  There is no CPU fallback.
 #include <cuda_runtime.h>
 
+#include <atomic>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -1150,8 +1151,165 @@ const char *ps_strerror(int code)
         case PS_ESTATE: return "coefficients not set: call ps_set_fraction first";
         case PS_ECUDA: return g_cuda_msg;
         case PS_ENOMEM: return "out of memory";
+        case PS_ETOOBIG:
+            return "grid too large for ps_residual_noalloc: more than PS_NOALLOC_MAX_CELLS "
+                   "(268435456) cells do not fit its fixed in-library scratch array";
         default: return "unknown error code";
     }
 }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------
+// ps_residual_noalloc: the residual norms for callers that must not allocate (see the header).
+//
+// ps_residual needs scratch memory beyond its inputs and outputs: one pair of partial sums per
+// 4096-cell chunk, which the final pass adds up.  It takes them from the context's workspace,
+// which somebody had to allocate.  The variant below keeps them in an array that is part of the
+// library image instead: every GPU that loads the library carries these 1 MiB + 256 B from the
+// moment the module is loaded until the process exits, and no call ever allocates or frees.
+namespace {
+
+constexpr int PS_NA_MAX_PARTS = (int)(PS_NOALLOC_MAX_CELLS / ps::RED_CHUNK);   // 65,536 chunks
+static_assert((long long)PS_NA_MAX_PARTS * ps::RED_CHUNK == PS_NOALLOC_MAX_CELLS, "whole chunks");
+constexpr int PS_NA_TAIL = 32;   // 256 bytes behind the partials; word 0 is the ticket counter
+
+// [0, MAX_PARTS): sum r^2 per chunk; [MAX_PARTS, 2 MAX_PARTS): sum rhs^2 per chunk; then the
+// ticket counter (blocks of the running call that have delivered their pair).  Shared by every
+// call on this device; holds whatever the last call left.
+static __device__ __align__(256) double ps_na_scratch[2 * PS_NA_MAX_PARTS + PS_NA_TAIL];
+
+// In host code `ps_na_scratch` is only a handle for the runtime, not an address a kernel could
+// use; the device address is asked for once per device and kept here.
+constexpr int PS_NA_MAX_DEVICES = 64;
+std::atomic<double *> g_na_scratch_dev[PS_NA_MAX_DEVICES];
+
+// One launch instead of ps_residual's two: every block reduces its chunk exactly as
+// ps_residual_partial(_pair)_kernel does and stores the pair in the scratch array; the block that
+// draws the last ticket then adds the pairs up in the order of ps_reduce_final_kernel (its 1024
+// threads and 32 warps are walked through by the 256 threads and 8 warps here), so the three
+// numbers are bitwise those of ps_residual.
+template <bool PAIR>
+__global__ void __launch_bounds__(ps::RED_THREADS)
+ps_residual_noalloc_kernel(ps::Grid g, const double *__restrict__ ax,
+                           const double *__restrict__ ay, const double *__restrict__ az,
+                           const double *__restrict__ rhs, const double *__restrict__ p,
+                           double *scratch, double *__restrict__ out)
+{
+    __shared__ double sm[2 * ps::FIN_THREADS / 32];
+    __shared__ int am_last;
+    double *partR2 = scratch, *partB2 = scratch + PS_NA_MAX_PARTS;
+    unsigned *ticket = reinterpret_cast<unsigned *>(scratch + 2 * PS_NA_MAX_PARTS);
+    const size_t N = g.cells();
+    const size_t base = (size_t)blockIdx.x * ps::RED_CHUNK;
+    double r2 = 0.0, b2 = 0.0;
+    if (PAIR) {
+#pragma unroll 2
+        for (int m = 0; m < ps::RED_CHUNK / (2 * ps::RED_THREADS); ++m) {
+            const size_t n = base + 2 * ((size_t)m * ps::RED_THREADS + threadIdx.x);
+            if (n < N) {
+                const int i = (int)((unsigned)n % (unsigned)g.nx);
+                const unsigned t = (unsigned)n / (unsigned)g.nx;
+                const int j = (int)(t % (unsigned)g.ny);
+                const int k = (int)(t / (unsigned)g.ny);
+                double2 b;
+                const double2 r = ps::residual_pair(g, ax, ay, az, rhs, p, i, j, k, n, b);
+                r2 = r2 + r.x * r.x;
+                r2 = r2 + r.y * r.y;
+                b2 = b2 + b.x * b.x;
+                b2 = b2 + b.y * b.y;
+            }
+        }
+    } else {
+#pragma unroll 4
+        for (int m = 0; m < ps::RED_CHUNK / ps::RED_THREADS; ++m) {
+            const size_t n = base + (size_t)m * ps::RED_THREADS + threadIdx.x;
+            if (n < N) {
+                const int i = (int)((unsigned)n % (unsigned)g.nx);
+                const unsigned t = (unsigned)n / (unsigned)g.nx;
+                const int j = (int)(t % (unsigned)g.ny);
+                const int k = (int)(t / (unsigned)g.ny);
+                const ps::Stencil s = ps::gather(g, ax, ay, az, p, i, j, k, n);
+                const double b = rhs[n];
+                const double r = ps::residual_at(s.axm, s.axp, s.aym, s.ayp, s.azm, s.azp, s.pxm,
+                                                 s.pxp, s.pym, s.pyp, s.pzm, s.pzp, p[n], b);
+                r2 = r2 + r * r;
+                b2 = b2 + b * b;
+            }
+        }
+    }
+    const double Rs = ps::block_tree_sum<ps::RED_THREADS>(r2, sm);
+    const double Bs = ps::block_tree_sum<ps::RED_THREADS>(b2, sm);
+    if (threadIdx.x == 0) {
+        __stcg(partR2 + blockIdx.x, Rs);
+        __stcg(partB2 + blockIdx.x, Bs);
+        __threadfence();                                  // the pair is visible before the ticket
+        am_last = atomicAdd(ticket, 1u) == gridDim.x - 1;
+    }
+    __syncthreads();
+    if (!am_last) return;
+    __threadfence();                                      // every other block's pair is visible now
+    const int nparts = (int)gridDim.x;
+    const int lane = threadIdx.x & 31;
+    double *smR = sm, *smB = sm + ps::FIN_THREADS / 32;
+    for (int vw = threadIdx.x >> 5; vw < ps::FIN_THREADS / 32; vw += ps::RED_THREADS / 32) {
+        double fr = 0.0, fb = 0.0;
+        for (int q = vw * 32 + lane; q < nparts; q += ps::FIN_THREADS) {
+            fr = fr + __ldcg(partR2 + q);
+            fb = fb + __ldcg(partB2 + q);
+        }
+        fr = ps::warp_tree_sum(fr);
+        fb = ps::warp_tree_sum(fb);
+        if (lane == 0) { smR[vw] = fr; smB[vw] = fb; }
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double R = 0.0, B = 0.0;
+#pragma unroll
+        for (int q = 0; q < ps::FIN_THREADS / 32; ++q) R = R + smR[q];
+#pragma unroll
+        for (int q = 0; q < ps::FIN_THREADS / 32; ++q) B = B + smB[q];
+        const double ra = sqrt(R), bn = sqrt(B);
+        out[0] = ra;
+        out[1] = (bn > 0.0) ? ra / bn : ra;
+        out[2] = bn;
+    }
+}
+
+}  // namespace
+
+extern "C" int ps_residual_noalloc(int nx, int ny, int nz, const double *ax_dev,
+                                   const double *ay_dev, const double *az_dev,
+                                   const double *rhs_dev, const double *p_dev, void *cuda_stream,
+                                   double *out_dev)
+{
+    if (nx < 1 || ny < 1 || nz < 2 || (nz & 1)) return PS_EINVAL;
+    if (!ax_dev || !ay_dev || !az_dev || !rhs_dev || !p_dev || !out_dev) return PS_EINVAL;
+    if (!aligned16(ax_dev, ay_dev, az_dev) || !aligned16(rhs_dev, p_dev) ||
+        ((uintptr_t)out_dev & 7u) != 0)
+        return PS_EINVAL;
+    if ((double)nx * (double)ny * (double)nz > (double)PS_NOALLOC_MAX_CELLS) return PS_ETOOBIG;
+    const ps::Grid g{nx, ny, nz};
+    int dev = -1;
+    PS_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= PS_NA_MAX_DEVICES) return PS_EINVAL;
+    // Set-up, once per device, with that device current: the device address of the array.
+    double *scratch = g_na_scratch_dev[dev].load(std::memory_order_acquire);
+    if (!scratch) {
+        PS_CUDA(cudaGetSymbolAddress((void **)&scratch, ps_na_scratch));
+        g_na_scratch_dev[dev].store(scratch, std::memory_order_release);
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    // The ticket counter must start at zero; the partials need no clearing (every slot the final
+    // pass reads is written by this launch first).  A memset node, not an allocation.
+    PS_CUDA(cudaMemsetAsync(scratch + 2 * PS_NA_MAX_PARTS, 0, PS_NA_TAIL * sizeof(double), st));
+    const int nparts = nparts_for(g.cells());
+    if (nx % 2 == 0)
+        ps_residual_noalloc_kernel<true><<<nparts, ps::RED_THREADS, 0, st>>>(
+            g, ax_dev, ay_dev, az_dev, rhs_dev, p_dev, scratch, out_dev);
+    else
+        ps_residual_noalloc_kernel<false><<<nparts, ps::RED_THREADS, 0, st>>>(
+            g, ax_dev, ay_dev, az_dev, rhs_dev, p_dev, scratch, out_dev);
+    PS_CUDA(cudaGetLastError());
+    return PS_OK;
+}
