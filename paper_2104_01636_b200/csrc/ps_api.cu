@@ -490,6 +490,9 @@ int ps_set_launch_options(ps_ctx *c, int dependent_launch, int pace_window)
         return PS_EINVAL;
     c->pdl_mode = dependent_launch;
     c->pace_mode = pace_window;
+    // forget an earlier "a CTA gave up waiting" (zm_pace): the caller asks for pacing afresh
+    if (c->fused.d_pace)
+        PS_CUDA(cudaMemsetAsync(c->fused.d_pace + 1, 0, sizeof(unsigned long long), c->stream));
     return PS_OK;
 }
 

@@ -145,31 +145,47 @@ def test_checks_notice_a_broken_protocol(torch_cuda, B, checked):
 
 def test_pacing_gives_up_instead_of_deadlocking(torch_cuda, B, checked, ora):
     """Pacing assumes that all CTAs of the persistent grid are resident at once.  If one of them
-    never shows up in the pacing counter (sabotage 2: CTA 0 does not claim its stages -- what a CTA
-    kept off the SMs by foreign work would look like) the others must not wait for ever: each gives
-    up after about a millisecond and runs free.  The launch ends, p is bitwise right, no ring
-    violation."""
+    never shows up in the pacing counter (sabotage 2: CTA 0 does not claim its stages until it
+    is done -- what a CTA kept off the SMs by foreign work looks like to the others) the others
+    must not wait for ever: each gives up after about a millisecond and runs free.  The give-up is
+    remembered on the device, so the launches after it do not wait at all; setting the launch
+    options again re-arms the pacing.  The paced launches come after an unpaced batch on the same
+    context: the host's base of the counter must not have moved during it (it once did, and no
+    paced launch after an unpaced one ever waited).  p is bitwise right, no ring violation."""
     import time
     w = workload(128, 128, 64)                     # 18 tiles x 1 z chunk: 18 CTAs of 67 stages;
                                                    # without CTA 0 the mean falls behind at stage 40
     coef = ora.coefficients(w.F, w.rho_l, w.rho_g, w.dx, w.dy, w.dz)
     p_ora = np.zeros_like(w.rhs)
-    ora.sweep(coef, w.rhs, p_ora, w.omega, 3)
+    ora.sweep(coef, w.rhs, p_ora, w.omega, 5)
     with B.PoissonSolver(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, lib=checked) as s:
         s.set_kernel(B.KERNEL_FUSED)
         s.set_tuning(1, 1)
         assert s.get_tuning()[3] == 18
-        s.set_launch_options(0, 2)
-        assert checked.ps_debug_sabotage(s._h, 2) == B.PS_OK
         s.set_fraction(dev(torch_cuda, w.F), w.rho_l, w.rho_g)
         rhs_d = dev(torch_cuda, w.rhs)
         p_d = torch_cuda.zeros_like(rhs_d)
-        torch_cuda.cuda.synchronize()
-        t0 = time.perf_counter()
-        s.sweeps(rhs_d, p_d, w.omega, 3)
-        torch_cuda.cuda.synchronize()
-        dt = time.perf_counter() - t0
-        assert 2e-3 < dt < 5.0, dt                   # 3 launches x (>= 1 ms of waiting + the sweep)
+        s.set_launch_options(0, 0)
+        s.sweeps(rhs_d, p_d, w.omega, 7)             # unpaced batch (and the warm-up)
+        p_d.zero_()
+        s.set_launch_options(0, 2)
+        assert checked.ps_debug_sabotage(s._h, 2) == B.PS_OK
+
+        def one_sweep():
+            torch_cuda.cuda.synchronize()
+            t0 = time.perf_counter()
+            s.sweeps(rhs_d, p_d, w.omega, 1)
+            torch_cuda.cuda.synchronize()
+            return time.perf_counter() - t0
+
+        t = [one_sweep() for _ in range(4)]
+        s.set_launch_options(0, 2)                   # re-arm
+        t.append(one_sweep())
+        free = min(t[1:4])
+        assert max(t) < 5.0, t
+        assert t[0] > free + 0.4e-3, t               # the first paced launch waited for CTA 0 ...
+        assert max(t[1:4]) < free + 0.3e-3, t        # ... the next three did not ...
+        assert t[4] > free + 0.4e-3, t               # ... and the re-armed one did again
         assert s.debug_read()[0] == 0, s.debug_read()
         assert int(np.count_nonzero(p_d.cpu().numpy() != p_ora)) == 0
 
