@@ -360,6 +360,15 @@ int ps_checked_build(void);
 int ps_debug_read(ps_ctx *c, unsigned long long *out_host);
 int ps_debug_sabotage(ps_ctx *c, int mode);
 
+/* Bandwidth probe for the roofline line of bench.py, no part of the solve path: out[i] = sum over
+ * r < reads of in[r*n + i], i < n, in one launch of `blocks` blocks of 512 threads with 16-byte
+ * streaming accesses.  reads = 5 is the fused sweep's mix (p, ax, ay, az, rhs in; p out), reads = 1
+ * a plain copy.  in_dev: reads*n doubles, out_dev: n doubles, both 16-byte aligned device memory of
+ * the caller; n even.  Asynchronous on cuda_stream (a cudaStream_t as void*); time it with events.
+ * PS_EINVAL: NULL / misaligned pointer, n odd or < 2, reads not in {1, 3, 5}, blocks < 1. */
+int ps_stream_probe(const double *in_dev, double *out_dev, size_t n, int reads, int blocks,
+                    void *cuda_stream);
+
 /* Kernels launched by this context since ps_create (bench.py's gpu_launches). */
 long long ps_launch_count(const ps_ctx *c);
 

@@ -44,7 +44,7 @@ SYMBOLS = ("ps_create", "ps_destroy", "ps_workspace_bytes", "ps_set_workspace", 
            "ps_checked_build", "ps_debug_read", "ps_debug_sabotage", "ps_timing", "ps_launch_count", "ps_strerror",
            "ps_mg_workspace_bytes", "ps_mg_set_workspace", "ps_mg_setup", "ps_mg_levels", "ps_mg_solve", "ps_mg_export_coarse",
            "ps_mg_residual_restrict", "ps_mg_prolong_add", "ps_rhs_from_velocity",
-           "ps_correct_velocity", "ps_face_divergence", "ps_ssf_rhs", "ps_residual_noalloc")
+           "ps_correct_velocity", "ps_face_divergence", "ps_ssf_rhs", "ps_residual_noalloc", "ps_stream_probe")
 
 
 class PsError(RuntimeError):
@@ -88,6 +88,7 @@ def load(path: str | None = None) -> ctypes.CDLL:
     if not os.path.exists(path):
         raise RuntimeError(f"{path} is missing: run `python -m paper_2104_01636_b200.build` "
                            "(the CUDA extension is the only compute path; there is no fallback)")
+    import torch  # noqa: F401  -- first, so that the library binds the libcudart torch loaded
     lib = ctypes.CDLL(path)
     vp, i, d, dp = ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.POINTER(ctypes.c_double)
     lib.ps_create.argtypes = [ctypes.POINTER(vp), i, i, i, d, d, d]
@@ -137,6 +138,7 @@ def load(path: str | None = None) -> ctypes.CDLL:
     lib.ps_face_divergence.argtypes = [vp, vp, vp, vp, vp, d, vp]
     lib.ps_ssf_rhs.argtypes = [vp, vp, vp, d, vp]
     lib.ps_residual_noalloc.argtypes = [i, i, i, vp, vp, vp, vp, vp, vp, vp]
+    lib.ps_stream_probe.argtypes = [vp, vp, ctypes.c_size_t, i, i, vp]
     lib.ps_strerror.argtypes = [i]
     lib.ps_strerror.restype = ctypes.c_char_p
     if path == _build.LIB:
@@ -194,6 +196,35 @@ def residual_noalloc(ax, ay, az, rhs, p, out, lib=None):
     _check(lib, lib.ps_residual_noalloc(nx, ny, nz, *ptrs, ctypes.c_void_p(s),
                                         ctypes.c_void_p(out.data_ptr())))
     return out
+
+
+def stream_probe_gbs(n: int, reads: int = 5, blocks_per_sm: int = 4, reps: int = 20,
+                     warmup: int = 3) -> float:
+    """GB/s (read + written bytes over CUDA-event time, mean of `reps` launches after `warmup`)
+    of ps_stream_probe on n doubles per stream: the library's own streaming kernel with the fused
+    sweep's 5-read / 1-write mix (reads=5) or a plain copy (reads=1).  A measured denominator for
+    bench.py's roofline beside the device-copy figure of MEASURED_PEAKS.json."""
+    import torch
+    lib = load()
+    n -= n & 1
+    src = torch.rand(reads * n, dtype=torch.float64, device="cuda")
+    dst = torch.empty(n, dtype=torch.float64, device="cuda")
+    blocks = blocks_per_sm * torch.cuda.get_device_properties(0).multi_processor_count
+    st = ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+    a, b = ctypes.c_void_p(src.data_ptr()), ctypes.c_void_p(dst.data_ptr())
+    for _ in range(warmup):
+        _check(lib, lib.ps_stream_probe(a, b, n, reads, blocks, st))
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(reps):
+        _check(lib, lib.ps_stream_probe(a, b, n, reads, blocks, st))
+    e1.record()
+    torch.cuda.synchronize()
+    if reads > 1:      # the probe really added the streams up
+        want = src.view(reads, n)[:, :1024].sum(0)
+        assert torch.allclose(dst[:1024], want, rtol=1e-14, atol=0)
+    return (reads + 1) * 8.0 * n * reps / (e0.elapsed_time(e1) * 1e-3) / 1e9
 
 
 def fused_plan(nx: int, ny: int, nz: int, sm_count: int = 148, z_chunks: int = 0):

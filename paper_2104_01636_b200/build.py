@@ -26,9 +26,14 @@ NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-std=c++17", "-O3", "--fmad=false", "-lineinfo",
     "-Xcompiler", "-fPIC", "-shared",
-    # the shared CUDA runtime (libcudart.so.12: torch's copy when torch is imported first, else the
-    # toolkit's through the rpath), so the shipped library carries none of the runtime's own code
-    "-cudart", "shared", "-Xlinker", "-rpath=/usr/local/cuda/lib64",
+    # the shared CUDA runtime (libcudart.so.12), so the shipped library carries none of the
+    # runtime's own code.  binding.load() imports torch first, so in a Python process the library
+    # binds the libcudart torch has already loaded (one runtime per process); a C program finds the
+    # toolkit's copy through the rpath _rpath_flags() adds.  Needs a CUDA 12 runtime (12.0 or later:
+    # cudaLaunchKernelEx with the cluster-dimension and programmatic-stream-serialization launch
+    # attributes, cudaGetDriverEntryPoint with its query-result argument); built and tested with
+    # the 12.9 toolkit against torch's 12.8 runtime.
+    "-cudart", "shared",
 ]
 
 
@@ -37,6 +42,17 @@ def _nvcc() -> str:
         if cand and os.path.exists(cand):
             return cand
     raise RuntimeError("nvcc not found: the CUDA path cannot be built (there is no CPU fallback)")
+
+
+def _rpath_flags(nvcc: str) -> list[str]:
+    """-rpath of the lib64 directory of the toolkit the resolved nvcc belongs to (not a fixed
+    /usr/local/cuda), for processes that have no libcudart loaded yet."""
+    home = os.environ.get("CUDA_HOME") or os.path.dirname(os.path.dirname(os.path.realpath(nvcc)))
+    for sub in ("lib64", os.path.join("targets", "x86_64-linux", "lib")):
+        d = os.path.join(home, sub)
+        if os.path.isdir(d):
+            return ["-Xlinker", f"-rpath={d}"]
+    return []
 
 
 def _deps():
@@ -56,7 +72,8 @@ def build(force: bool = False, verbose: bool = False, checked: bool = False) -> 
     if not force and up_to_date(lib):
         return lib
     tmp = f"{lib}.{os.getpid()}.tmp"
-    cmd = [_nvcc(), *NVCC_FLAGS, *(["-DPS_CHECKED"] if checked else []),
+    nvcc = _nvcc()
+    cmd = [nvcc, *NVCC_FLAGS, *_rpath_flags(nvcc), *(["-DPS_CHECKED"] if checked else []),
            *(["-Xptxas", "-v"] if verbose else []),
            "-o", tmp, *[os.path.join(_CSRC, s) for s in SOURCES]]
     res = subprocess.run(cmd, cwd=_CSRC, capture_output=True, text=True)

@@ -1146,6 +1146,24 @@ int ps_ssf_rhs(ps_ctx *c, const double *F_dev, const double *kappa_dev, double s
     return PS_OK;
 }
 
+int ps_stream_probe(const double *in_dev, double *out_dev, size_t n, int reads, int blocks,
+                    void *cuda_stream)
+{
+    if (!in_dev || !out_dev || n < 2 || (n & 1) || blocks < 1 || !aligned16(in_dev, out_dev))
+        return PS_EINVAL;
+    const double2 *in = reinterpret_cast<const double2 *>(in_dev);
+    double2 *out = reinterpret_cast<double2 *>(out_dev);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    switch (reads) {
+        case 1: ps::ps_stream_probe_kernel<1><<<blocks, 512, 0, st>>>(in, out, n / 2); break;
+        case 3: ps::ps_stream_probe_kernel<3><<<blocks, 512, 0, st>>>(in, out, n / 2); break;
+        case 5: ps::ps_stream_probe_kernel<5><<<blocks, 512, 0, st>>>(in, out, n / 2); break;
+        default: return PS_EINVAL;
+    }
+    PS_CUDA(cudaGetLastError());
+    return PS_OK;
+}
+
 const char *ps_strerror(int code)
 {
     switch (code) {

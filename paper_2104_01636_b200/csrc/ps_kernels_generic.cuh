@@ -354,4 +354,43 @@ ps_reduce_final_kernel(const double *__restrict__ partR2, const double *__restri
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Bandwidth probe with the sweep's read:write mix (bench.py's second roofline denominator): out =
+// sum of READS input streams, 16-byte accesses, two elements of every stream in flight per
+// thread.  The fused sweep reads five streams (p, ax, ay, az, rhs) and writes one; a device copy
+// (the MEASURED_PEAKS.json figure) reads one and writes one, and HBM turns around between reads and
+// writes less often in the first case.  No part of the solve path.
+template <int READS>
+__global__ void __launch_bounds__(512)
+ps_stream_probe_kernel(const double2 *__restrict__ in, double2 *__restrict__ out, size_t n2)
+{
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    for (; q + stride < n2; q += 2 * stride) {
+        double2 a[READS], b[READS];
+#pragma unroll
+        for (int r = 0; r < READS; ++r) {
+            a[r] = __ldcs(in + (size_t)r * n2 + q);
+            b[r] = __ldcs(in + (size_t)r * n2 + q + stride);
+        }
+        double2 sa = a[0], sb = b[0];
+#pragma unroll
+        for (int r = 1; r < READS; ++r) {
+            sa.x = sa.x + a[r].x; sa.y = sa.y + a[r].y;
+            sb.x = sb.x + b[r].x; sb.y = sb.y + b[r].y;
+        }
+        __stcs(out + q, sa);
+        __stcs(out + q + stride, sb);
+    }
+    if (q < n2) {
+        double2 sa = __ldcs(in + q);
+#pragma unroll
+        for (int r = 1; r < READS; ++r) {
+            const double2 v = __ldcs(in + (size_t)r * n2 + q);
+            sa.x = sa.x + v.x; sa.y = sa.y + v.y;
+        }
+        __stcs(out + q, sa);
+    }
+}
+
 }  // namespace ps

@@ -150,6 +150,69 @@ def write_traffic(raw_csv: str, key: str, source: str, path: str) -> dict:
     return rec
 
 
+SASS_OPCODES = ("UTMALDG", "UTMAPF", "SYNCS.ARRIVE", "SYNCS.PHASECHK", "SYNCS.EXCH", "UCGABAR",
+                "ACQBULK", "PREEXIT", "DFMA", "DMUL", "DADD", "MUFU.RCP64H", "LDG*.128",
+                "LDG*.64", "STG*.128", "STG*.64", "LDS", "STS", "ATOMG", "RED", "SHFL", "BAR.SYNC",
+                "NANOSLEEP", "HMMA", "UTCHMMA", "UTCQMMA")      # A*.w: opcode A of width w
+
+
+def sass_summary() -> str:
+    """Markdown: the architectures in the built product library (`cuobjdump -lelf`) and, per
+    kernel, how often the instructions that tell a Blackwell-native tile-movement kernel from a
+    recompiled one occur in its SASS (`cuobjdump -sass`): TMA tensor loads (UTMALDG), mbarrier
+    arrive / try-wait (SYNCS.*), the cluster barrier (UCGABAR_*), the dependent-launch pair
+    (ACQBULK, PREEXIT), the fp64 arithmetic and the 16-byte global accesses.  No GPU needed."""
+    import hashlib
+    import re
+    import subprocess
+    from . import build
+    lib = build.build()
+    elf = subprocess.run(["cuobjdump", "-lelf", lib], capture_output=True, text=True, check=True).stdout
+    sass = subprocess.run(["cuobjdump", "-sass", lib], capture_output=True, text=True, check=True).stdout
+    demangle = {}
+    names = re.findall(r"Function : (\S+)", sass)
+    out = subprocess.run(["cu++filt", *names], capture_output=True, text=True)
+    if out.returncode == 0:
+        demangle = dict(zip(names, out.stdout.splitlines()))
+    kernels, cur = {}, None
+    for line in sass.splitlines():
+        m = re.search(r"Function : (\S+)", line)
+        if m:
+            cur = kernels.setdefault(m.group(1), {"n": 0, **{k: 0 for k in SASS_OPCODES}})
+            continue
+        m = re.match(r"\s+/\*[0-9a-f]{4,}\*/\s+(?:@!?U?P\d+\s+)?([A-Z][A-Z0-9_.]+)", line)
+        if m and cur is not None:
+            cur["n"] += 1
+            op = m.group(1)
+            for k in SASS_OPCODES:
+                head, star, width = k.partition("*")
+                if op.startswith(head) and (not star or width in op):
+                    cur[k] += 1
+    used = [k for k in SASS_OPCODES if any(v[k] for v in kernels.values())]
+    absent = [k for k in SASS_OPCODES if k not in used]
+    srcs = sorted(build._deps())
+    h = hashlib.sha256()
+    for f in srcs:
+        with open(f, "rb") as fh:
+            h.update(fh.read())
+    md = ["# SASS of libps_poisson.so: architectures and instruction counts per kernel", "",
+          "Command: `python -m paper_2104_01636_b200.report --sass` (runs `cuobjdump -lelf` and "
+          "`cuobjdump -sass` on the library built from the committed sources; no GPU).",
+          f"sha256 over the library's sources (include/ps_poisson.h, csrc/*): `{h.hexdigest()[:16]}`.",
+          "", "`cuobjdump -lelf`:", "", "```", elf.strip(), "```", "",
+          "Instruction counts (prefix match on the opcode; columns that are zero everywhere are "
+          "listed below the table):", "",
+          "| kernel | instr | " + " | ".join(used) + " |", "|---|---:|" + "---:|" * len(used)]
+    for name, c in sorted(kernels.items(), key=lambda kv: -kv[1]["n"]):
+        short = re.sub(r"\((int|bool)\)", "", demangle.get(name, name))
+        short = re.sub(r"\(.*", "", short)
+        short = re.sub(r"<unnamed>::|ps::|void ", "", short)
+        md.append(f"| `{short}` | {c['n']} | " + " | ".join(str(c[k]) for k in used) + " |")
+    md += ["", "Absent from every kernel: " + (", ".join(absent) or "-") +
+           " (no tensor-core instruction: the path is a stencil, not a contraction).", ""]
+    return "\n".join(md)
+
+
 def to_markdown(rows) -> str:
     head = ("| cfg | workload | kernel | sweeps | ms | Gcell-upd/s | model GB/s | res_rel after | "
             "SOR to 1e-8: sweeps | seconds | res_rel | MG to 1e-8: cycles (levels) | seconds | res_rel |\n"
@@ -190,7 +253,17 @@ def main(argv=None):
                          "DRAM bytes per launch to profiles/traffic.json (no GPU needed)")
     ap.add_argument("--traffic-key", default="fused:config4")
     ap.add_argument("--traffic-source", default="", help="where the capture is summarised")
+    ap.add_argument("--sass", action="store_true",
+                    help="only print the architecture list and per-kernel instruction counts of "
+                         "the built library (cuobjdump; no GPU needed)")
     args = ap.parse_args(argv)
+    if args.sass:
+        md = sass_summary()
+        print(md)
+        if args.md:
+            with open(args.md, "w") as f:
+                f.write(md)
+        return
     if args.traffic_from:
         import os
         root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))

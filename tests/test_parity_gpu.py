@@ -603,3 +603,27 @@ def test_edge_shapes_all_variants_and_default_multigrid(torch_cuda, B, ora, shap
         q_d = torch_cuda.zeros_like(rhs_d)
         s.mg_solve(rhs_d, q_d, 2, 0.0)
         assert_p_parity(q_d.cpu().numpy(), q_ora, f"{shape} default multigrid")
+
+
+# ---------------------------------------------------------------- bench.py's bandwidth probe
+@pytest.mark.parametrize("reads", [1, 3, 5])
+def test_stream_probe_adds_its_streams(torch_cuda, B, reads):
+    """ps_stream_probe (the second roofline denominator of bench.py) reads every element of every
+    stream and writes every output: ragged sizes, more and fewer elements than threads."""
+    import ctypes
+    torch = torch_cuda
+    lib = B.load()
+    for n, blocks in ((2, 1), (1026, 1), (100_000, 3), (3_000_002, 592)):
+        src = torch.rand(reads * n, dtype=torch.float64, device="cuda")
+        dst = torch.full((n + 2,), -1.0, dtype=torch.float64, device="cuda")
+        rc = lib.ps_stream_probe(ctypes.c_void_p(src.data_ptr()), ctypes.c_void_p(dst.data_ptr()),
+                                 n, reads, blocks, None)
+        assert rc == B.PS_OK
+        torch.cuda.synchronize()
+        want = src[:n].clone()
+        for r in range(1, reads):
+            want += src[r * n:(r + 1) * n]
+        assert torch.equal(dst[:n], want), (n, blocks)
+        assert float(dst[n]) == -1.0 and float(dst[n + 1]) == -1.0
+    assert lib.ps_stream_probe(None, None, 4, 5, 1, None) == B.PS_EINVAL
+    assert B.stream_probe_gbs(1 << 22, 5, reps=2, warmup=1) > 0.0
