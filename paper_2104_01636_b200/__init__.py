@@ -6,4 +6,4 @@ The compute path is hand-written CUDA for sm_100a behind the C ABI of include/ps
 fallback: using the solver without the built library raises.  `workload` is the seeded input
 generator (numpy, host side) and is importable on its own.
 """
-__all__ = ["workload", "binding", "build", "replicas", "report", "mg_tune", "sanitize"]
+__all__ = ["workload", "binding", "build", "replicas", "report"]
