@@ -156,7 +156,8 @@ class _MgParams(ctypes.Structure):
                 ("nu_growth", ctypes.c_int), ("nu_max", ctypes.c_int),
                 ("coarse_sweeps", ctypes.c_int), ("gamma", ctypes.c_int),
                 ("omega_s", ctypes.c_double), ("omega_c", ctypes.c_double),
-                ("nu_max_deep", ctypes.c_int)]
+                ("nu_max_deep", ctypes.c_int), ("stall_cycles", ctypes.c_int),
+                ("omega_c_step", ctypes.c_double)]
 
 
 def _mg_lib():
@@ -218,15 +219,17 @@ def mg_max_levels(nx: int, ny: int, nz: int) -> int:
 def mg_solve(coef, rhs: np.ndarray, p: np.ndarray, max_cycles: int, tol: float, levels: int = 99,
              nu1: int = 2, nu2: int = 2, coarse_sweeps: int = 50, gamma: int = 1,
              omega_s: float = 1.2, nu_growth: int = 1, nu_max: int = 1 << 20,
-             omega_c: float | None = None, nu_max_deep: int | None = None) -> Info:
+             omega_c: float | None = None, nu_max_deep: int | None = None,
+             stall_cycles: int = 0, omega_c_step: float = 0.0) -> Info:
     """M5 + M6 in place on p; Info.sweeps holds the number of cycles.  omega_s relaxes level 0,
     omega_c the levels below it (None: the same factor everywhere); nu_max_deep caps the
-    smoothing count from level 2 on (None: nu_max on every level)."""
+    smoothing count from level 2 on (None: nu_max on every level); stall_cycles / omega_c_step:
+    the safeguard M7 (0: off)."""
     ax, ay, az = coef
     nx, ny, nz = _shape(p)
     prm = _MgParams(levels, nu1, nu2, nu_growth, nu_max, coarse_sweeps, gamma, omega_s,
                     omega_s if omega_c is None else omega_c,
-                    nu_max if nu_max_deep is None else nu_max_deep)
+                    nu_max if nu_max_deep is None else nu_max_deep, stall_cycles, omega_c_step)
     info = _Info()
     rc = _mg_lib().ora_mg_solve(nx, ny, nz, _p(ax), _p(ay), _p(az), _p(rhs), _p(p),
                                 ctypes.byref(prm), max_cycles, tol, ctypes.byref(info))

@@ -352,10 +352,25 @@ int ora_mg_solve(int nx, int ny, int nz, const double *ax, const double *ay, con
     double ra = 0.0, rr = 0.0, bn = 0.0;
     int c = 0, converged = 0;
     if (ok) {
+        /* M7: the cycle is a fixed linear iteration; with omega_c close to 2 it can diverge on
+         * operators it was not tuned on (strongly anisotropic spacing).  The only remedy taken is
+         * the one stated in ora_mg_params: a lower omega_c for the cycles that follow. */
+        ora_mg_params q = *prm;
+        double best = 0.0;
+        int have_best = 0, stall = 0;
         for (c = 1; c <= max_cycles; ++c) {
-            mg_cycle(lv, 0, nlev, prm);
+            mg_cycle(lv, 0, nlev, &q);
             ora_residual(nx, ny, nz, ax, ay, az, rhs, p, &ra, &rr, &bn);
             if (tol > 0.0 && rr <= tol) { converged = 1; break; }
+            if (q.stall_cycles > 0) {
+                if (!have_best || rr < best) {
+                    best = rr; have_best = 1; stall = 0;
+                } else if (++stall >= q.stall_cycles) {
+                    q.omega_c = q.omega_c - q.omega_c_step;
+                    if (q.omega_c < 1.0) q.omega_c = 1.0;
+                    best = rr; stall = 0;
+                }
+            }
         }
         if (c > max_cycles) c = max_cycles;
         if (max_cycles == 0) ora_residual(nx, ny, nz, ax, ay, az, rhs, p, &ra, &rr, &bn);

@@ -45,6 +45,12 @@ typedef struct {
                           * solver (DESIGN.md §12 M6) */
     int nu_max_deep;     /* cap of the per-level smoothing count on the levels l >= 2 (level 1 is
                           * capped by nu_max alone); values >= nu_max change nothing */
+    int stall_cycles;    /* DESIGN.md §12 M7 (safeguard of ora_mg_solve, not part of a cycle): > 0:
+                          * once this many cycles in a row have ended with a norm that is not below
+                          * the best norm so far, omega_c is lowered by omega_c_step (never below
+                          * 1) for the cycles that follow, that norm becomes the new best and the
+                          * count restarts; 0: omega_c stays as given */
+    double omega_c_step; /* >= 0 */
 } ora_mg_params;
 
 void ora_mg_coarsen(int nx, int ny, int nz, const double *ax, const double *ay, const double *az,

@@ -310,3 +310,78 @@ def test_deep_levels_have_their_own_cap(ora):
     d = np.zeros_like(rhs)
     ora.mg_solve(coef, rhs, d, 2, 0.0, **dict(kw, nu_max=4))          # 2, 4, 4, 4: level 1 bound too
     assert not np.array_equal(d, p)
+
+
+# ------------------------------------------------------------------ M7 (safeguard of the solve loop)
+ANISO = dict(levels=6, nu1=0, nu2=2, coarse_sweeps=10, gamma=1, omega_s=1.4, omega_c=1.97,
+             nu_growth=24, nu_max=48, nu_max_deep=48)
+
+
+def _aniso_case(ora):
+    w = wl.make_custom(16, 16, 32, 2, 8, 5, dx=4 / 16, dy=1 / 16, dz=1 / 16)   # spacing 4:1:1
+    return w, ora.coefficients(w.F, w.rho_l, w.rho_g, w.dx, w.dy, w.dz)
+
+
+def test_stall_safeguard_is_the_stated_bookkeeping_around_unchanged_cycles(ora):
+    """M7 changes no cycle, only which omega_c the next one runs with.  One ora_mg_solve call with
+    stall_cycles = 3, omega_c_step = 0.05 on a duct with 4:1:1 spacing (where omega_c = 1.97
+    diverges) must equal, bitwise, single cycles (max_cycles = 1, safeguard off: the pinned
+    cycle) strung together by hand with the rule as ora_mg_params states it: a norm below the best
+    so far resets the count; the third norm in a row that is not lowers omega_c by the step, makes
+    that norm the new best and restarts the count."""
+    w, coef = _aniso_case(ora)
+    ncyc = 30
+    p = np.zeros_like(w.rhs)
+    info = ora.mg_solve(coef, w.rhs, p, ncyc, 0.0, stall_cycles=3, omega_c_step=0.05, **ANISO)
+    q = np.zeros_like(w.rhs)
+    prm = dict(ANISO)
+    best, stall, lowered, norms = None, 0, [], []
+    for c in range(1, ncyc + 1):
+        one = ora.mg_solve(coef, w.rhs, q, 1, 0.0, **prm)
+        norms.append(one.res_rel)
+        if best is None or one.res_rel < best:
+            best, stall = one.res_rel, 0
+        else:
+            stall += 1
+            if stall == 3:
+                prm["omega_c"] = max(prm["omega_c"] - 0.05, 1.0)
+                best, stall = one.res_rel, 0
+                lowered.append(c)
+    assert lowered, "the case must trigger the safeguard"
+    assert lowered[0] >= 4                       # never before three non-improving norms
+    assert np.array_equal(p, q)
+    assert info.sweeps == ncyc and info.res_rel == norms[-1]
+    # and it does what it is for: the plain cycle diverges here, the safeguarded one comes down
+    r = np.zeros_like(w.rhs)
+    plain = ora.mg_solve(coef, w.rhs, r, ncyc, 0.0, **ANISO)
+    assert plain.res_rel > 1.0 > 0.05 > info.res_rel
+
+
+def test_stall_safeguard_off_and_floor(ora):
+    """stall_cycles = 0 is the cycle loop as it was (omega_c_step ignored); a converging run never
+    triggers the safeguard (config-1-like duct, defaults: same p with and without); omega_c is
+    never lowered below 1."""
+    w, coef = _aniso_case(ora)
+    a, b = np.zeros_like(w.rhs), np.zeros_like(w.rhs)
+    ora.mg_solve(coef, w.rhs, a, 8, 0.0, **ANISO)
+    ora.mg_solve(coef, w.rhs, b, 8, 0.0, stall_cycles=0, omega_c_step=0.5, **ANISO)
+    assert np.array_equal(a, b)
+    # floor: a step of 5 lands on omega_c = 1 after the first trigger, never below
+    c, d = np.zeros_like(w.rhs), np.zeros_like(w.rhs)
+    ora.mg_solve(coef, w.rhs, c, 12, 0.0, stall_cycles=1, omega_c_step=5.0, **ANISO)
+    prm = dict(ANISO)
+    best = None
+    for _ in range(12):
+        one = ora.mg_solve(coef, w.rhs, d, 1, 0.0, **prm)
+        if best is None or one.res_rel < best:
+            best = one.res_rel
+        else:
+            prm["omega_c"], best = 1.0, one.res_rel
+    assert prm["omega_c"] == 1.0 and np.array_equal(c, d)
+    # a healthy run: isotropic duct, nothing to safeguard
+    v = wl.make_custom(16, 16, 32, 2, 8, 5)
+    cv = ora.coefficients(v.F, v.rho_l, v.rho_g, v.dx, v.dy, v.dz)
+    e, f = np.zeros_like(v.rhs), np.zeros_like(v.rhs)
+    i1 = ora.mg_solve(cv, v.rhs, e, 40, 1e-8, **ANISO)
+    i2 = ora.mg_solve(cv, v.rhs, f, 40, 1e-8, stall_cycles=3, omega_c_step=0.05, **ANISO)
+    assert i1.converged and i2.converged and i1.sweeps == i2.sweeps and np.array_equal(e, f)
