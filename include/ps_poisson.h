@@ -277,6 +277,16 @@ typedef struct {
                          /* and coarsest solver), in (0,2)                                     */
     int nu_max_deep;     /* cap of the per-level count on the levels l >= 2 (>= 1; level 1 is  */
                          /* capped by nu_max alone; values >= nu_max change nothing)           */
+    int stall_cycles;    /* safeguard of ps_mg_solve (M7), >= 0.  The cycle is a  */
+                         /* fixed linear iteration and an omega_c close to 2 can diverge on     */
+                         /* operators it was not tuned on (strongly anisotropic spacing).  > 0: */
+                         /* once this many cycles in a row have ended with a norm that is not   */
+                         /* below the best norm of the call so far, omega_c is lowered by       */
+                         /* omega_c_step (never below 1) for the cycles that follow, that norm  */
+                         /* becomes the new best and the count restarts.  0: never.  A          */
+                         /* converging solve never triggers it; each ps_mg_solve call starts    */
+                         /* from the omega_c of ps_mg_setup again                               */
+    double omega_c_step; /* >= 0, finite                                                       */
 } ps_mg_params;
 
 /* Device memory of the coarse levels (per level: coefficients, ping-pong buffer, reduction

@@ -31,8 +31,11 @@ KERNEL_NAMES = {KERNEL_AUTO: "auto", KERNEL_TWOPASS: "twopass", KERNEL_FUSED: "f
 # omega_c = 1.98 is ~10 % faster and 1.985 still converges on every config and seed tried; 1.99 does
 # not on all.  The one place they are written down: bench.py, report.py and the parity tests take
 # them from here.
+# stall_cycles / omega_c_step: the safeguard M7 -- the defaults are tuned on isotropic bubbly ducts
+# and omega_c = 1.97 diverges on 4:1:1 or 1:2:4 spacing; three cycles in a row without a new best
+# norm lower omega_c by 0.05 (tests/test_mg_heldout_gpu.py, profiles/r03_mg_heldout.md).
 MG_DEFAULTS = dict(levels=6, nu1=0, nu2=2, coarse_sweeps=10, gamma=1, omega_s=1.4, omega_c=1.97,
-                   nu_growth=24, nu_max=48, nu_max_deep=48)
+                   nu_growth=24, nu_max=48, nu_max_deep=48, stall_cycles=3, omega_c_step=0.05)
 
 # every symbol include/ps_poisson.h declares (tests check the library exports each one)
 SYMBOLS = ("ps_create", "ps_destroy", "ps_workspace_bytes", "ps_set_workspace", "ps_set_stream",
@@ -58,7 +61,8 @@ class _MgParams(ctypes.Structure):
                 ("nu_growth", ctypes.c_int), ("nu_max", ctypes.c_int),
                 ("coarse_sweeps", ctypes.c_int), ("gamma", ctypes.c_int),
                 ("omega_s", ctypes.c_double), ("omega_c", ctypes.c_double),
-                ("nu_max_deep", ctypes.c_int)]
+                ("nu_max_deep", ctypes.c_int), ("stall_cycles", ctypes.c_int),
+                ("omega_c_step", ctypes.c_double)]
 
 
 class _Info(ctypes.Structure):
@@ -389,7 +393,8 @@ class PoissonSolver:
                  coarse_sweeps: int | None = None, gamma: int | None = None,
                  omega_s: float | None = None, nu_growth: int | None = None,
                  nu_max: int | None = None, omega_c: float | None = None,
-                 nu_max_deep: int | None = None) -> int:
+                 nu_max_deep: int | None = None, stall_cycles: int | None = None,
+                 omega_c_step: float | None = None) -> int:
         """Build the level hierarchy from the current coefficients; returns the levels in use.
         With no arguments: MG_DEFAULTS.  Any argument given replaces its default, except that
         omega_c follows an explicitly given omega_s when it is not given itself (one relaxation
@@ -402,13 +407,14 @@ class PoissonSolver:
             nu_max_deep = nu_max
         given = dict(levels=levels, nu1=nu1, nu2=nu2, coarse_sweeps=coarse_sweeps, gamma=gamma,
                      omega_s=omega_s, omega_c=omega_c, nu_growth=nu_growth, nu_max=nu_max,
-                     nu_max_deep=nu_max_deep)
+                     nu_max_deep=nu_max_deep, stall_cycles=stall_cycles,
+                     omega_c_step=omega_c_step)
         q = dict(MG_DEFAULTS)
         q.update({k: v for k, v in given.items() if v is not None})
         levels = q["levels"]
         prm = _MgParams(q["levels"], q["nu1"], q["nu2"], q["nu_growth"], q["nu_max"],
                         q["coarse_sweeps"], q["gamma"], q["omega_s"], q["omega_c"],
-                        q["nu_max_deep"])
+                        q["nu_max_deep"], q["stall_cycles"], q["omega_c_step"])
         if self._torch_owns:               # the level memory is a torch allocation too
             need = self._lib.ps_mg_workspace_bytes(self._h, levels)
             if need and (self._mg_ws is None or self._mg_ws[0].numel() < need + 256):

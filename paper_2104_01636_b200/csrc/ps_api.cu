@@ -959,7 +959,8 @@ int ps_mg_setup(ps_ctx *c, const ps_mg_params *prm)
         prm->nu_max_deep < 1 ||
         prm->coarse_sweeps < 1 || prm->gamma < 1 ||
         prm->gamma > 2 || !(prm->omega_s > 0.0 && prm->omega_s < 2.0) ||
-        !(prm->omega_c > 0.0 && prm->omega_c < 2.0))
+        !(prm->omega_c > 0.0 && prm->omega_c < 2.0) || prm->stall_cycles < 0 ||
+        !(prm->omega_c_step >= 0.0) || !std::isfinite(prm->omega_c_step))
         return PS_EINVAL;
     if (!c->have_coef) return PS_ESTATE;
     int dev = -1;
@@ -998,6 +999,22 @@ int ps_mg_solve(ps_ctx *c, const double *rhs_dev, double *p_dev, int max_cycles,
     if (!c->have_coef || !c->mg_ready) return PS_ESTATE;
     for (ps_ctx *k = c->child; k; k = k->child) k->stream = c->stream;
     int cyc = 0, converged = 0, rc = 0;
+    // Safeguard M7: the parameters of this call; omega_c is lowered by
+    // omega_c_step (never below 1) once stall_cycles cycles in a row have ended with a norm that
+    // is not below the best so far.  Same bookkeeping, in the same order, as the oracle's loop.
+    ps_mg_params q = c->mgp;
+    double best = 0.0;
+    int have_best = 0, stall = 0;
+    auto safeguard = [&](double rr) {
+        if (q.stall_cycles <= 0) return;
+        if (!have_best || rr < best) {
+            best = rr; have_best = 1; stall = 0;
+        } else if (++stall >= q.stall_cycles) {
+            q.omega_c = q.omega_c - q.omega_c_step;
+            if (q.omega_c < 1.0) q.omega_c = 1.0;
+            best = rr; stall = 0;
+        }
+    };
     if (mg_fused_norm_ok(c) && max_cycles > 0) {
         // (cycle, check)* as below, but the check of cycle n rides on the residual + restriction
         // pass that opens cycle n + 1 (one pass of 41 B/cell instead of 40 + 41); the pass after
@@ -1009,8 +1026,9 @@ int ps_mg_solve(ps_ctx *c, const double *rhs_dev, double *p_dev, int max_cycles,
                 PS_CUDA(cudaStreamSynchronize(c->stream));
                 if (tol > 0.0 && c->h_scal[1] <= tol) { converged = 1; break; }
                 if (cyc == max_cycles || !std::isfinite(c->h_scal[1])) break;
+                safeguard(c->h_scal[1]);
             }
-            if ((rc = mg_cycle(c, c->mgp, rhs_dev, p_dev, 0, true))) return rc;
+            if ((rc = mg_cycle(c, q, rhs_dev, p_dev, 0, true))) return rc;
         }
         if (info) {
             info->sweeps = cyc;
@@ -1022,11 +1040,12 @@ int ps_mg_solve(ps_ctx *c, const double *rhs_dev, double *p_dev, int max_cycles,
         return PS_OK;
     }
     for (cyc = 1; cyc <= max_cycles; ++cyc) {
-        if ((rc = mg_cycle(c, c->mgp, rhs_dev, p_dev))) return rc;
+        if ((rc = mg_cycle(c, q, rhs_dev, p_dev))) return rc;
         if ((rc = enqueue_residual(c, rhs_dev, p_dev))) return rc;
         PS_CUDA(cudaStreamSynchronize(c->stream));
         if (tol > 0.0 && c->h_scal[1] <= tol) { converged = 1; break; }
         if (!std::isfinite(c->h_scal[1])) break;
+        safeguard(c->h_scal[1]);
     }
     if (cyc > max_cycles) cyc = max_cycles;
     if (max_cycles == 0) {

@@ -210,7 +210,7 @@ def test_diverging_parameters_stop_early(torch_cuda, B):
     with B.PoissonSolver(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz) as s:
         s.set_fraction(dev(torch_cuda, w.F), w.rho_l, w.rho_g)
         s.mg_setup(levels=6, nu1=0, nu2=2, coarse_sweeps=30, gamma=1, omega_s=1.9, omega_c=1.9,
-                   nu_growth=4, nu_max=16)
+                   nu_growth=4, nu_max=16, stall_cycles=0)      # safeguard M7 off: let it diverge
         p_d = torch_cuda.zeros(w.rhs.shape, dtype=torch_cuda.float64, device="cuda")
         info = s.mg_solve(dev(torch_cuda, w.rhs), p_d, 100000, 1e-8)
         assert not info.converged and info.sweeps < 100000
@@ -266,3 +266,37 @@ def test_level_memory_is_caller_owned_and_setup_failures_leave_no_half_built_hie
         p_d = torch_cuda.zeros(w.rhs.shape, dtype=torch_cuda.float64, device="cuda")
         s.mg_solve(dev(torch_cuda, w.rhs), p_d, 2, 0.0)
         same(p_d.cpu().numpy(), p_o, "library-owned level memory")
+
+
+# ---------------------------------------------------------------- M7: safeguard of the solve loop
+@pytest.mark.parametrize("h", [(4 / 64, 1 / 64, 1 / 64), (1 / 64, 2 / 64, 4 / 64)])
+def test_stall_safeguard_bitwise_on_anisotropic_ducts(torch_cuda, B, ora, h):
+    """The binding defaults on a duct with 4:1:1 / 1:2:4 spacing: omega_c = 1.97 diverges there,
+    the safeguard (3 cycles without a new best norm -> omega_c - 0.05) brings it back.  Both the
+    fused-norm loop (nu1 = 0: the defaults) and the plain loop (nu1 = 1) must take the oracle's
+    decisions: p bitwise after 40 cycles, and without the safeguard the same run diverges."""
+    w = workload(64, 64, 128, 6, 8, h)
+    coef = ora.coefficients(w.F, w.rho_l, w.rho_g, w.dx, w.dy, w.dz)
+    rhs_d = dev(torch_cuda, w.rhs)
+    with B.PoissonSolver(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz) as s:
+        s.set_fraction(dev(torch_cuda, w.F), w.rho_l, w.rho_g)
+        for extra in ({}, {"nu1": 1}):
+            prm = dict(B.MG_DEFAULTS, **extra)
+            p_o = np.zeros_like(w.rhs)
+            io = ora.mg_solve(coef, w.rhs, p_o, 40, 0.0, **prm)
+            s.mg_setup(**prm)
+            p_d = torch_cuda.zeros_like(rhs_d)
+            ig = s.mg_solve(rhs_d, p_d, 40, 0.0)
+            same(p_d.cpu().numpy(), p_o, f"safeguarded cycles {extra}")
+            assert abs(ig.res_rel - io.res_rel) <= 1e-10 * io.res_rel
+            assert ig.res_rel < 0.1
+        s.mg_setup(**dict(B.MG_DEFAULTS, stall_cycles=0))
+        p_d = torch_cuda.zeros_like(rhs_d)
+        plain = s.mg_solve(rhs_d, p_d, 40, 0.0)
+        assert plain.res_rel > 10 * ig.res_rel
+        lib = B.load()
+        bad = B._MgParams(6, 0, 2, 24, 48, 10, 1, 1.4, 1.97, 48, -1, 0.05)
+        import ctypes
+        assert lib.ps_mg_setup(s._h, ctypes.byref(bad)) == B.PS_EINVAL
+        bad = B._MgParams(6, 0, 2, 24, 48, 10, 1, 1.4, 1.97, 48, 3, float("nan"))
+        assert lib.ps_mg_setup(s._h, ctypes.byref(bad)) == B.PS_EINVAL
